@@ -1,0 +1,119 @@
+"""ctypes loader for the CPU oracle (TEST INFRASTRUCTURE — see oracle/euler_oracle.cpp header).
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs import
+this package.  It imports nothing from paper_1204_4779_b200 (the CUDA path) and vice versa.
+"""
+import ctypes
+import os
+
+import numpy as np
+
+from . import build as _build
+
+_LIBS = {}
+_DT = {np.dtype(np.float32): 0, np.dtype(np.float64): 1}
+
+
+def _lib(kind="serial"):
+    if kind not in _LIBS:
+        path = _build.build()[kind]
+        L = ctypes.CDLL(path)
+        vp, i64, dbl, cint = ctypes.c_void_p, ctypes.c_int64, ctypes.c_double, ctypes.c_int
+        L.oracle_create.restype = vp
+        L.oracle_create.argtypes = [cint, ctypes.POINTER(i64), ctypes.POINTER(dbl), dbl, cint]
+        L.oracle_destroy.argtypes = [vp]
+        L.oracle_destroy.restype = None
+        L.oracle_set_option.argtypes = [vp, ctypes.c_char_p, i64]
+        L.oracle_set_state.argtypes = [vp, vp]
+        L.oracle_get_state.argtypes = [vp, vp]
+        L.oracle_cfl_dt.argtypes = [vp, dbl]
+        L.oracle_cfl_dt.restype = dbl
+        L.oracle_step.argtypes = [vp, dbl]
+        L.oracle_stage.argtypes = [vp, dbl, vp]
+        L.oracle_run.argtypes = [vp, dbl, i64, dbl, ctypes.POINTER(i64), ctypes.POINTER(dbl)]
+        L.oracle_riemann.argtypes = [cint, cint, cint, cint, dbl, vp, vp, vp]
+        L.oracle_minbee.argtypes = [cint, dbl, dbl, dbl, ctypes.POINTER(dbl), ctypes.POINTER(dbl)]
+        L.oracle_num_threads.restype = cint
+        _LIBS[kind] = L
+    return _LIBS[kind]
+
+
+class Oracle:
+    """One oracle solver instance.  State arrays are (nf, [nz,] [ny,] nx), x fastest."""
+
+    def __init__(self, n, extent, gamma, dtype, boundary="periodic", riemann="hllc", threads="serial"):
+        self.n = tuple(int(v) for v in n)  # x first
+        self.dims = len(self.n)
+        self.dtype = np.dtype(dtype)
+        self.nf = self.dims + 2
+        self.shape = (self.nf,) + tuple(reversed(self.n))
+        self._L = _lib(threads)
+        narr = (ctypes.c_int64 * self.dims)(*self.n)
+        earr = (ctypes.c_double * self.dims)(*[float(e) for e in extent])
+        self._h = self._L.oracle_create(self.dims, narr, earr, float(gamma), _DT[self.dtype])
+        if not self._h:
+            raise ValueError("oracle_create failed")
+        self._opt("boundary", {"periodic": 0, "outflow": 1}[boundary])
+        self._opt("riemann", {"hllc": 0, "hll": 1}[riemann])
+
+    def _opt(self, key, val):
+        if self._L.oracle_set_option(self._h, key.encode(), val) != 0:
+            raise ValueError(f"bad option {key}={val}")
+
+    def set_state(self, U):
+        U = np.ascontiguousarray(U, dtype=self.dtype)
+        assert U.shape == self.shape, (U.shape, self.shape)
+        self._L.oracle_set_state(self._h, U.ctypes.data)
+
+    def get_state(self):
+        out = np.empty(self.shape, self.dtype)
+        self._L.oracle_get_state(self._h, out.ctypes.data)
+        return out
+
+    def cfl_dt(self, cfl):
+        return self._L.oracle_cfl_dt(self._h, float(cfl))
+
+    def step(self, dt):
+        self._L.oracle_step(self._h, float(dt))
+
+    def stage(self, tau):
+        out = np.empty(self.shape, self.dtype)
+        self._L.oracle_stage(self._h, float(tau), out.ctypes.data)
+        return out
+
+    def run(self, cfl, nsteps, t_end=0.0):
+        k = ctypes.c_int64(0)
+        t = ctypes.c_double(0)
+        self._L.oracle_run(self._h, float(cfl), int(nsteps), float(t_end), ctypes.byref(k), ctypes.byref(t))
+        return k.value, t.value
+
+    def close(self):
+        if self._h:
+            self._L.oracle_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def riemann(VL, VR, axis, gamma, dims, dtype=np.float64, kind="hllc"):
+    VL = np.ascontiguousarray(VL, np.float64)
+    VR = np.ascontiguousarray(VR, np.float64)
+    F = np.empty(dims + 2, np.float64)
+    rc = _lib().oracle_riemann(_DT[np.dtype(dtype)], dims, axis, {"hllc": 0, "hll": 1}[kind], float(gamma),
+                               VL.ctypes.data, VR.ctypes.data, F.ctypes.data)
+    assert rc == 0
+    return F
+
+
+def minbee(y0, y1, y2, dtype=np.float64):
+    lo, hi = ctypes.c_double(), ctypes.c_double()
+    _lib().oracle_minbee(_DT[np.dtype(dtype)], y0, y1, y2, ctypes.byref(lo), ctypes.byref(hi))
+    return lo.value, hi.value
+
+
+def num_threads(kind="omp"):
+    return _lib(kind).oracle_num_threads()

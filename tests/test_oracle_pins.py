@@ -1,0 +1,364 @@
+"""Pins for the CPU oracle (no GPU): what the paper and the mathematics fix, independent of the oracle.
+
+P1 uniform state bitwise · P2 conservation · P3 closed-form N=8 Sod half-stage (golden) ·
+P4 stationary contact · P5 Sod vs exact Riemann solution (golden star values) · P6 entropy wave
+(Eq. 28) order -> 2 · P7 sound wave (Eq. 29) · P8 x/y/z embedding bitwise · P9 mirror
+symmetry · P10 Riemann-solver special cases · P11 independent NumPy restatement on tiny grids ·
+P12 robustness of the BASELINE configs at reduced size.  Numbering follows SURVEY.md §8(c3).
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+import exact_riemann
+import numpy_scheme
+from paper_1204_4779_b200 import inputs
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def golden(name):
+    out = {}
+    for line in open(os.path.join(HERE, "golden", name)):
+        line = line.strip()
+        if line and not line.startswith("#"):
+            k, v = line.split()
+            out[k] = float(v)
+    return out
+
+
+def make(oracle_mod, w, riemann="hllc", threads="serial", boundary=None):
+    o = oracle_mod.Oracle(w.n, w.extent, w.gamma, w.dtype, boundary or w.boundary, riemann, threads)
+    o.set_state(w.U)
+    return o
+
+
+def uniform_state(n, dtype, v):
+    dims = len(n)
+    shape = tuple(reversed(n))
+    rho = np.full(shape, 1.3)
+    p = np.full(shape, 0.7)
+    vel = [np.full(shape, v[b]) for b in range(dims)]
+    return np.ascontiguousarray(inputs.conserved_from_primitive(rho, vel, p, 1.4).astype(dtype))
+
+
+# ---------------------------------------------------------------- P1
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("riemann", ["hllc", "hll"])
+@pytest.mark.parametrize("boundary", ["periodic", "outflow"])
+@pytest.mark.parametrize("n", [(9,), (6, 5), (5, 4, 6)])
+def test_p1_uniform_state_is_bitwise_fixed(oracle_mod, n, boundary, riemann, dtype):
+    U = uniform_state(n, dtype, (0.37, -1.9, 2.3))  # supersonic in y,z, subsonic in x
+    o = oracle_mod.Oracle(n, [1.0] * len(n), 1.4, dtype, boundary, riemann)
+    o.set_state(U)
+    for _ in range(5):
+        o.step(o.cfl_dt(0.4))
+    assert np.array_equal(o.get_state(), U)
+
+
+# ---------------------------------------------------------------- P2
+@pytest.mark.parametrize("dtype,tol", [(np.float64, 1e-14), (np.float32, 1e-6)])
+@pytest.mark.parametrize("n", [(64,), (24, 20), (12, 10, 14)])
+def test_p2_conservation_on_periodic_grids(oracle_mod, n, dtype, tol):
+    w = inputs.random_smooth(n, dtype, seed=5)
+    o = make(oracle_mod, w)
+    s0 = [math.fsum(f.ravel().astype(np.float64)) for f in w.U]
+    scale = [math.fsum(np.abs(f.ravel().astype(np.float64))) for f in w.U]
+    o.run(0.4, 100)
+    U = o.get_state()
+    assert np.all(np.isfinite(U))
+    assert not np.array_equal(U, w.U)
+    for f in range(w.nf):
+        drift = abs(math.fsum(U[f].ravel().astype(np.float64)) - s0[f]) / scale[f]
+        assert drift < tol, (f, drift)
+
+
+# ---------------------------------------------------------------- P3
+def sod8(dtype=np.float64, mirror=False):
+    x = (np.arange(8) + 0.5) / 8
+    left = (x > 0.5) if mirror else (x < 0.5)
+    rho, p = np.where(left, 1.0, 0.125), np.where(left, 1.0, 0.1)
+    return np.ascontiguousarray(np.stack([rho, 0 * rho, p / 0.4]).astype(dtype))
+
+
+@pytest.mark.parametrize("riemann", ["hllc", "hll"])
+def test_p3_closed_form_first_half_stage(oracle_mod, riemann):
+    g = golden("sod_n8_first_stage.txt")
+    cL = math.sqrt(1.4)
+    # the golden numbers are themselves the closed forms of the header
+    assert g["c_L"] == pytest.approx(cL, rel=1e-15)
+    assert g["dt"] == pytest.approx(0.4 / (8 * cL), rel=1e-15)
+    assert g["hllc_F_rho"] == pytest.approx(4 / 11 * cL, rel=1e-15)
+    assert g["hllc_F_m"] == pytest.approx(27 / 55, rel=1e-15)
+    assert g["hllc_F_E"] == pytest.approx(54 / 55 * cL, rel=1e-15)
+    assert g["hll_F_rho"] == pytest.approx(7 / 16 * cL, rel=1e-15)
+    assert g["hll_F_E"] == pytest.approx(9 / 8 * cL, rel=1e-15)
+
+    o = oracle_mod.Oracle((8,), (1.0,), 1.4, np.float64, "outflow", riemann)
+    U0 = sod8()
+    o.set_state(U0)
+    dt = o.cfl_dt(0.4)
+    assert dt == pytest.approx(g["dt"], rel=2e-16)
+    F = oracle_mod.riemann([1, 0, 1], [0.125, 0, 0.1], 0, 1.4, 1, np.float64, riemann)
+    for k, name in enumerate(["rho", "m", "E"]):
+        assert F[k] == pytest.approx(g[f"{riemann}_F_{name}"], rel=4e-16)
+    U1 = o.stage(0.5 * dt)
+    for k, name in enumerate(["rho", "m", "E"]):
+        assert U1[k, 3] == pytest.approx(g[f"{riemann}_U1_3_{name}"], rel=1e-15)
+        assert U1[k, 4] == pytest.approx(g[f"{riemann}_U1_4_{name}"], rel=1e-15)
+    # every other cell is untouched by the first stage
+    keep = [0, 1, 2, 5, 6, 7]
+    assert np.array_equal(U1[:, keep], U0[:, keep])
+
+
+@pytest.mark.parametrize("riemann", ["hllc", "hll"])
+def test_p3_mirrored_problem_gives_mirrored_fluxes(oracle_mod, riemann):
+    F = oracle_mod.riemann([1, 0, 1], [0.125, 0, 0.1], 0, 1.4, 1, np.float64, riemann)
+    Fm = oracle_mod.riemann([0.125, 0, 0.1], [1, 0, 1], 0, 1.4, 1, np.float64, riemann)
+    assert Fm[0] == pytest.approx(-F[0], rel=1e-15)
+    assert Fm[1] == pytest.approx(F[1], rel=1e-15)
+    assert Fm[2] == pytest.approx(-F[2], rel=1e-15)
+
+
+# ---------------------------------------------------------------- P4
+def test_p4_stationary_contact_hllc_exact_hll_smears(oracle_mod):
+    n = 32
+    x = (np.arange(n) + 0.5) / n
+    rho = np.where(x < 0.5, 1.0, 0.125)
+    U0 = np.stack([rho, 0 * rho, np.full(n, 1.0 / 0.4)])
+    res = {}
+    for riemann in ("hllc", "hll"):
+        o = oracle_mod.Oracle((n,), (1.0,), 1.4, np.float64, "outflow", riemann)
+        o.set_state(U0)
+        o.step(o.cfl_dt(0.4))
+        one = o.get_state()
+        o.run(0.4, 99)
+        res[riemann] = (one, o.get_state())
+    assert np.abs(res["hllc"][1] - U0).max() < 1e-14
+    # HLL has no contact wave: it diffuses the jump already in the first step
+    assert np.abs(res["hll"][0][0] - U0[0]).max() > 1e-2
+
+
+# ---------------------------------------------------------------- P5
+def test_p5_exact_star_values_match_golden():
+    g = golden("sod_exact_star.txt")
+    L, R, gam = (1.0, 0.0, 1.0), (0.125, 0.0, 0.1), 1.4
+    ps, us = exact_riemann.star_state(L, R, gam)
+    assert ps == pytest.approx(g["p_star"], rel=1e-13)
+    assert us == pytest.approx(g["u_star"], rel=1e-13)
+    rsl = ps ** (1 / gam)
+    assert rsl == pytest.approx(g["rho_star_L"], rel=1e-13)
+    cR = math.sqrt(gam * 0.1 / 0.125)
+    shock = cR * math.sqrt(2.4 / 2.8 * ps / 0.1 + 0.4 / 2.8)
+    assert shock == pytest.approx(g["shock_speed"], rel=1e-13)
+    for t in (0.2, 0.125):
+        assert 0.5 - math.sqrt(1.4) * t == pytest.approx(g[f"t{t}_rarefaction_head"], abs=1e-6)
+        assert 0.5 + (us - g["c_star_L"]) * t == pytest.approx(g[f"t{t}_rarefaction_tail"], abs=1e-6)
+        assert 0.5 + us * t == pytest.approx(g[f"t{t}_contact"], abs=1e-6)
+        assert 0.5 + shock * t == pytest.approx(g[f"t{t}_shock"], abs=1e-6)
+
+
+@pytest.mark.parametrize("riemann", ["hllc", "hll"])
+def test_p5_sod_converges_to_exact_solution(oracle_mod, riemann):
+    L, R, gam = (1.0, 0.0, 1.0), (0.125, 0.0, 0.1), 1.4
+    errs, steps = [], []
+    for n in (64, 128, 256, 512):
+        w = inputs.sod(n)
+        o = make(oracle_mod, w, riemann)
+        k, t = o.run(w.cfl, w.steps, w.t_end)
+        assert t == 0.2
+        steps.append(k)
+        rho = o.get_state()[0]
+        assert np.all(np.isfinite(rho)) and rho.min() > 0.12 and rho.max() < 1.0 + 1e-12
+        exact = exact_riemann.cell_averaged_density(n, 0.2, L, R, gam)
+        errs.append(np.abs(rho - exact).mean())
+    # L1 error falls monotonically, at the ~first-order rate a limited scheme has on discontinuities
+    for a, b in zip(errs, errs[1:]):
+        assert 0.45 * a < b < 0.72 * a, errs
+    # sanity ranges from SURVEY.md §8(c3) P5 (indicative values, HLLC): 1.02e-2 ... 1.85e-3; 279 steps at N=256
+    assert 8e-3 < errs[0] < 1.3e-2 and 1.4e-3 < errs[3] < 2.4e-3, errs
+    assert 270 <= steps[2] <= 290, steps
+
+
+# ---------------------------------------------------------------- P6 / P7 (the paper's own tests)
+def _l1_after_one_period(oracle_mod, n, kind, riemann="hllc"):
+    x = (np.arange(n) + 0.5) / n
+    g = 1.4
+    if kind == "entropy":  # PAPER.md Eq. 28
+        rho, v, p = 2.0 + np.sin(2 * np.pi * x), np.ones(n), np.ones(n)
+    else:  # PAPER.md Eq. 29, A = 1e-5
+        A = 1e-5
+        s = np.sin(2 * np.pi * x)
+        rho, v, p = g * (1 + A * s), A * s, 1 + g * A * s
+    U0 = inputs.conserved_from_primitive(rho, [v], p, g)
+    o = oracle_mod.Oracle((n,), (1.0,), g, np.float64, "periodic", riemann)
+    o.set_state(U0)
+    k, t = o.run(0.4, 10**7, 1.0)
+    assert t == 1.0
+    return np.abs(o.get_state()[0] - rho).mean()
+
+
+def test_p6_entropy_wave_second_order(oracle_mod):
+    ns = [32, 64, 128, 256, 512]
+    e = [_l1_after_one_period(oracle_mod, n, "entropy") for n in ns]
+    orders = [math.log2(a / b) for a, b in zip(e, e[1:])]
+    assert all(b > a for a, b in zip(orders, orders[1:])), orders  # rising towards 2
+    assert orders[-1] > 1.7 and orders[-2] > 1.7, orders
+    assert all(o < 2.2 for o in orders), orders
+    assert 3e-2 < e[0] < 9e-2 and 2e-4 < e[-1] < 8e-4, e  # SURVEY §8(c3) P6 indicative range
+
+
+def test_p7_sound_wave_returns_after_one_period(oracle_mod):
+    ns = [32, 64, 128, 256]
+    e = [_l1_after_one_period(oracle_mod, n, "sound") for n in ns]
+    orders = [math.log2(a / b) for a, b in zip(e, e[1:])]
+    assert orders[-1] > 1.7, orders
+    assert e[-1] < 5e-8, e  # amplitude of the wave is 1.4e-5: the error is a small fraction of it
+    # a wrong sound speed (e.g. dropped pressure term) leaves an O(A) error at every resolution
+    assert e[0] < 0.2 * 1.4e-5, e
+
+
+# ---------------------------------------------------------------- P8
+@pytest.mark.parametrize("riemann", ["hllc", "hll"])
+@pytest.mark.parametrize("dims,axis", [(2, 0), (2, 1), (3, 0), (3, 1), (3, 2)])
+def test_p8_embedding_is_bitwise_identical(oracle_mod, dims, axis, riemann):
+    n = 24
+    w1 = inputs.sod(n)
+    o1 = make(oracle_mod, w1, riemann)
+    wd = inputs.sod(n, dims=dims, axis=axis, n_other=4)
+    od = make(oracle_mod, wd, riemann)
+    for _ in range(6):
+        dt1, dtd = o1.cfl_dt(0.4), od.cfl_dt(0.4)
+        assert dt1 == dtd
+        o1.step(dt1)
+        od.step(dtd)
+    U1, Ud = o1.get_state(), od.get_state()
+    ax = dims - 1 - axis  # array axis (after the field axis) of the embedded direction
+    Ud = np.moveaxis(Ud, 1 + ax, -1)  # (f, other..., n)
+    for f1, fd in ((0, 0), (1, 1 + axis), (2, dims + 1)):
+        assert np.array_equal(Ud[fd], np.broadcast_to(U1[f1], Ud[fd].shape))
+    for b in range(dims):
+        if b != axis:
+            assert np.all(Ud[1 + b] == 0)
+
+
+# ---------------------------------------------------------------- P9
+@pytest.mark.parametrize("riemann", ["hllc", "hll"])
+def test_p9_mirror_symmetry(oracle_mod, riemann):
+    w = inputs.random_smooth((40, 28), np.float64, seed=11)
+    o = make(oracle_mod, w, riemann)
+    Um = w.U[:, :, ::-1].copy()
+    Um[1] *= -1  # x -> -x, v_x -> -v_x
+    om = oracle_mod.Oracle(w.n, w.extent, w.gamma, w.dtype, "periodic", riemann)
+    om.set_state(Um)
+    for _ in range(10):
+        dt, dtm = o.cfl_dt(0.4), om.cfl_dt(0.4)
+        assert dt == pytest.approx(dtm, rel=1e-15)
+        o.step(dt)
+        om.step(dt)
+    A, B = o.get_state(), om.get_state()[:, :, ::-1].copy()
+    B[1] *= -1
+    for f in range(4):
+        assert np.abs(A[f] - B[f]).max() <= 1e-13 * np.abs(A[f]).max()
+
+
+# ---------------------------------------------------------------- P10
+@pytest.mark.parametrize("kind", ["hllc", "hll"])
+@pytest.mark.parametrize("dims,axis", [(1, 0), (2, 0), (2, 1), (3, 0), (3, 1), (3, 2)])
+def test_p10_consistency_and_supersonic_upwinding(oracle_mod, dims, axis, kind):
+    g = 5.0 / 3.0
+    rng = np.random.default_rng(7)
+    for trial in range(20):
+        V = np.concatenate([[rng.uniform(0.1, 3)], rng.uniform(-2, 2, dims), [rng.uniform(0.1, 3)]])
+        rho, v, p = V[0], V[1 : 1 + dims], V[-1]
+        E = p / (g - 1) + 0.5 * rho * v @ v
+        Fphys = np.concatenate([[rho * v[axis]], rho * v[axis] * v + p * (np.arange(dims) == axis), [v[axis] * (E + p)]])
+        # VL = VR  =>  the physical flux (to rounding)
+        F = oracle_mod.riemann(V, V, axis, g, dims, np.float64, kind)
+        assert np.allclose(F, Fphys, rtol=1e-13, atol=1e-13)
+        # supersonic to the right: F = F(VL) whatever VR is (and mirrored)
+        c = math.sqrt(g * p / rho)
+        VL = V.copy()
+        VL[1 + axis] = 3.0 * c + 1.0
+        VR = VL.copy()
+        VR[0] *= 0.9
+        VR[-1] *= 0.8
+        vL = VL[1 : 1 + dims]
+        EL = VL[-1] / (g - 1) + 0.5 * VL[0] * vL @ vL
+        FL = np.concatenate([[VL[0] * vL[axis]], VL[0] * vL[axis] * vL + VL[-1] * (np.arange(dims) == axis),
+                             [vL[axis] * (EL + VL[-1])]])
+        assert np.allclose(oracle_mod.riemann(VL, VR, axis, g, dims, np.float64, kind), FL, rtol=1e-14, atol=0)
+
+
+def test_p10_minbee_cases(oracle_mod):
+    # Eq. 21: opposite signs -> 0; otherwise the smaller one-sided difference
+    assert oracle_mod.minbee(1.0, 2.0, 1.5) == (2.0, 2.0)
+    assert oracle_mod.minbee(1.0, 2.0, 4.0) == (1.5, 2.5)  # dy01 = 1 < dy12 = 2
+    assert oracle_mod.minbee(0.0, 2.0, 3.0) == (1.5, 2.5)  # dy12 = 1 < dy01 = 2
+    assert oracle_mod.minbee(3.0, 2.0, 0.0) == (2.5, 1.5)  # negative slopes
+    assert oracle_mod.minbee(2.0, 2.0, 5.0) == (2.0, 2.0)  # one zero difference -> zero slope
+    assert oracle_mod.minbee(1.0, 2.0, 3.0) == (1.5, 2.5)  # tie -> dy12 (same value)
+
+
+# ---------------------------------------------------------------- P11
+@pytest.mark.parametrize("kind", ["hllc", "hll"])
+@pytest.mark.parametrize("boundary", ["periodic", "outflow"])
+@pytest.mark.parametrize("n", [(8,), (7,), (4, 4), (6, 5), (4, 4, 4), (5, 4, 6)])
+def test_p11_matches_independent_numpy_restatement(oracle_mod, n, boundary, kind):
+    w = inputs.random_smooth(n, np.float64, seed=3 + len(n), gamma=1.4, boundary=boundary)
+    o = make(oracle_mod, w, kind)
+    dr = [e / m for e, m in zip(w.extent, w.n)]
+    U = w.U.astype(np.float64)
+    for _ in range(3):
+        dt = o.cfl_dt(0.4)
+        assert dt == pytest.approx(numpy_scheme.cfl_dt(U, 0.4, dr, w.gamma), rel=1e-14)
+        o.step(dt)
+        U = numpy_scheme.step(U, dt, dr, w.gamma, boundary, kind)
+        got = o.get_state()
+        for f in range(w.nf):
+            assert np.abs(got[f] - U[f]).max() <= 2e-14 * np.abs(U[f]).max(), (f, n)
+
+
+def test_p11_sod_many_steps_against_numpy(oracle_mod):
+    # all four Riemann-fan branches and the limiter at a moving shock, 60 steps on 8 cells... and 64 cells
+    for n in (8, 64):
+        w = inputs.sod(n)
+        o = make(oracle_mod, w, "hllc")
+        U = w.U.copy()
+        for _ in range(60):
+            dt = o.cfl_dt(0.4)
+            o.step(dt)
+            U = numpy_scheme.step(U, dt, [1.0 / n], 1.4, "outflow", "hllc")
+        assert np.abs(o.get_state() - U).max() < 1e-12
+
+
+# ---------------------------------------------------------------- P12
+@pytest.mark.parametrize("riemann", ["hllc", "hll"])
+def test_p12_baseline_configs_are_robust_at_reduced_size(oracle_mod, riemann):
+    w = inputs.kelvin_helmholtz(128, dtype=np.float32, seed=0, steps=100)
+    o = make(oracle_mod, w, riemann, threads="omp")
+    dt0 = o.cfl_dt(w.cfl)
+    assert 1.0e-3 < dt0 < 1.6e-3  # ~6.6e-4 at 256^2, scales with 1/N
+    o.run(w.cfl, 100)
+    U = o.get_state()
+    assert np.all(np.isfinite(U)) and U[0].min() > 0.9 and U[0].max() < 2.1
+
+    w = inputs.blast(32, np.float32, seed=2, steps=50)
+    o = make(oracle_mod, w, riemann, threads="omp")
+    assert 0.55 < w.U[0].min() and w.U[0].max() < 1.7
+    o.run(w.cfl, 50)
+    U = o.get_state()
+    assert np.all(np.isfinite(U)) and U[0].min() > 0.05 and U[0].max() < 3.0
+    V = numpy_scheme.prim(U.astype(np.float64), w.gamma)
+    assert V[4].min() > 0.5
+
+
+def test_omp_build_is_bit_identical_to_serial(oracle_mod):
+    w = inputs.random_smooth((20, 12, 9), np.float32, seed=2)
+    a, b = make(oracle_mod, w, threads="serial"), make(oracle_mod, w, threads="omp")
+    ka = a.run(0.3, 7)
+    kb = b.run(0.3, 7)
+    assert ka == kb
+    assert np.array_equal(a.get_state(), b.get_state())
