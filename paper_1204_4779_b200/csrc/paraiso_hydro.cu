@@ -1,0 +1,553 @@
+// paraiso_hydro.cu — C-ABI entry points (include/paraiso_hydro.h), handle, device buffers, variant
+// dispatch and CUDA-graph replay.  Host code only orchestrates: every step of the path runs in the
+// kernels of hydro_kernels_*.cuh.  No CPU fallback exists.
+#include "../../include/paraiso_hydro.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+
+#include "hydro_kernels_basic.cuh"
+#include "hydro_kernels_fused.cuh"
+
+using namespace ph;
+
+enum { VARIANT_FUSED = 0, VARIANT_MANIFEST_FLUX = 1, VARIANT_MANIFEST_ALL = 2, VARIANT_DELAYED = 3 };
+
+struct paraiso_hydro {
+  int dims = 0, dtype = 0, nf = 0;
+  int64_t n[3] = {1, 1, 1};
+  int64_t N = 0;
+  double extent[3] = {1, 1, 1};
+  double gamma = 0;
+  size_t esize = 0;
+
+  int boundary = BOUNDARY_PERIODIC, riemann = RIEMANN_HLLC, variant = VARIANT_FUSED;
+  int block[3] = {0, 0, 0};
+  int tile_depth = 0, cells_per_thread = 0, use_graph = 1;
+
+  void* U[2] = {nullptr, nullptr};  // U[0]: current state / U_base; U[1]: stage-1 result
+  void* V = nullptr;                // manifest_all: primitives
+  void* LO[3] = {nullptr, nullptr, nullptr};
+  void* HI[3] = {nullptr, nullptr, nullptr};
+  void* F[3] = {nullptr, nullptr, nullptr};   // manifest_*: face fluxes
+  void* Fb[3] = {nullptr, nullptr, nullptr};  // outflow boundary faces
+  Scalars* sc = nullptr;
+  cudaStream_t stream = nullptr;
+  bool has_state = false;
+  int64_t launches = 0;
+
+  cudaGraphExec_t graph_exec = nullptr;
+  int graph_key = -1;  // option fingerprint the graph was captured with
+  int graph_steps = 0;
+
+  std::string err;
+};
+
+static thread_local std::string g_create_error = "no error";
+
+static int fail(paraiso_hydro* h, int code, const std::string& msg) {
+  if (h)
+    h->err = msg;
+  else
+    g_create_error = msg;
+  return code;
+}
+
+#define CUDA_TRY(h, expr)                                                                              \
+  do {                                                                                                 \
+    cudaError_t e_ = (expr);                                                                           \
+    if (e_ != cudaSuccess)                                                                             \
+      return fail(h, e_ == cudaErrorMemoryAllocation ? PARAISO_ENOMEM : PARAISO_ECUDA,                 \
+                  std::string(#expr) + ": " + cudaGetErrorString(e_));                                 \
+  } while (0)
+
+template <class Real>
+static Geom<Real> make_geom(const paraiso_hydro* h) {
+  Geom<Real> g;
+  for (int a = 0; a < 3; ++a) {
+    g.n[a] = int(h->n[a]);
+    g.dr[a] = a < h->dims ? Real(h->extent[a] / double(h->n[a])) : Real(1);
+    g.idr[a] = a < h->dims ? Real(double(h->n[a]) / h->extent[a]) : Real(0);
+  }
+  g.N = h->N;
+  g.gamma = Real(h->gamma);
+  g.gm1 = g.gamma - Real(1);
+  g.igm1 = Real(1) / g.gm1;
+  g.boundary = h->boundary;
+  return g;
+}
+
+static void free_intermediates(paraiso_hydro* h) {
+  cudaFree(h->V);
+  h->V = nullptr;
+  for (int a = 0; a < 3; ++a) {
+    cudaFree(h->LO[a]);
+    cudaFree(h->HI[a]);
+    cudaFree(h->F[a]);
+    cudaFree(h->Fb[a]);
+    h->LO[a] = h->HI[a] = h->F[a] = h->Fb[a] = nullptr;
+  }
+}
+
+static void drop_graph(paraiso_hydro* h) {
+  if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
+  h->graph_exec = nullptr;
+  h->graph_key = -1;
+}
+
+// Manifest intermediates are allocated on first use of a Manifest variant.
+static int ensure_intermediates(paraiso_hydro* h) {
+  const size_t field_bytes = size_t(h->nf) * h->N * h->esize;
+  if (h->variant == VARIANT_MANIFEST_ALL || h->variant == VARIANT_MANIFEST_FLUX) {
+    for (int a = 0; a < h->dims; ++a) {
+      if (!h->F[a]) CUDA_TRY(h, cudaMalloc(&h->F[a], field_bytes));
+      if (!h->Fb[a]) CUDA_TRY(h, cudaMalloc(&h->Fb[a], size_t(h->nf) * (h->N / h->n[a]) * h->esize));
+    }
+  }
+  if (h->variant == VARIANT_MANIFEST_ALL) {
+    if (!h->V) CUDA_TRY(h, cudaMalloc(&h->V, field_bytes));
+    for (int a = 0; a < h->dims; ++a) {
+      if (!h->LO[a]) CUDA_TRY(h, cudaMalloc(&h->LO[a], field_bytes));
+      if (!h->HI[a]) CUDA_TRY(h, cudaMalloc(&h->HI[a], field_bytes));
+    }
+  }
+  return PARAISO_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Stage launchers.  stage 1: U[0] -> U[1] (tau = dt/2); stage 2: U[1] (+ own-cell U[0]) -> U[0] in place.
+template <class Real, int D, int RS>
+struct Launch {
+  static unsigned int grid1d(int64_t N, int bs) { return (unsigned int)((N + bs - 1) / bs); }
+
+  template <int A>
+  static void recon_riemann(paraiso_hydro* h, const Geom<Real>& g) {
+    const int bs = 256;
+    const unsigned int gs = grid1d(h->N, bs);
+    k_recon<Real, D, A><<<gs, bs, 0, h->stream>>>((const Real*)h->V, (Real*)h->LO[A], (Real*)h->HI[A], g, h->sc);
+    k_riemann<Real, D, A, RS>
+        <<<gs, bs, 0, h->stream>>>((const Real*)h->LO[A], (const Real*)h->HI[A], (Real*)h->F[A], (Real*)h->Fb[A], g, h->sc);
+    h->launches += 2;
+  }
+  template <int A>
+  static void flux(paraiso_hydro* h, const Geom<Real>& g, const Real* Uin) {
+    const int bs = 128;
+    k_flux<Real, D, A, RS><<<grid1d(h->N, bs), bs, 0, h->stream>>>(Uin, (Real*)h->F[A], (Real*)h->Fb[A], g, h->sc);
+    h->launches += 1;
+  }
+
+  template <int STAGE>
+  static void update(paraiso_hydro* h, const Geom<Real>& g, Real* Uout) {
+    FluxArrays<Real, D> fa;
+    for (int a = 0; a < 3; ++a) {
+      fa.F[a] = (const Real*)h->F[a];
+      fa.Fb[a] = (const Real*)h->Fb[a];
+    }
+    const int bs = 256;
+    k_update<Real, D, STAGE><<<grid1d(h->N, bs), bs, 0, h->stream>>>((const Real*)h->U[0], Uout, fa, g, h->sc);
+    h->launches += 1;
+  }
+
+  template <int STAGE>
+  static void stage(paraiso_hydro* h) {
+    const Geom<Real> g = make_geom<Real>(h);
+    const Real* Uin = (const Real*)(STAGE == 1 ? h->U[0] : h->U[1]);
+    Real* Uout = (Real*)(STAGE == 1 ? h->U[1] : h->U[0]);
+    switch (h->variant) {
+      case VARIANT_MANIFEST_ALL: {
+        const int bs = 256;
+        k_prim<Real, D><<<grid1d(h->N, bs), bs, 0, h->stream>>>(Uin, (Real*)h->V, g, h->sc);
+        h->launches += 1;
+        recon_riemann<0>(h, g);
+        if constexpr (D > 1) recon_riemann<1>(h, g);
+        if constexpr (D > 2) recon_riemann<2>(h, g);
+        update<STAGE>(h, g, Uout);
+        break;
+      }
+      case VARIANT_MANIFEST_FLUX: {
+        flux<0>(h, g, Uin);
+        if constexpr (D > 1) flux<1>(h, g, Uin);
+        if constexpr (D > 2) flux<2>(h, g, Uin);
+        update<STAGE>(h, g, Uout);
+        break;
+      }
+      case VARIANT_FUSED:
+        if (launch_fused_stage<Real, D, RS, STAGE>(Uin, (const Real*)h->U[0], Uout, g, h->sc, h->stream, h->block,
+                                                   h->tile_depth, h->cells_per_thread)) {
+          h->launches += 1;
+          break;
+        }
+        // 1-D grids (and shapes the marching kernel does not cover) use the Delayed kernel: fall through
+      default: {
+        const int bs = h->block[0] > 0 ? h->block[0] : 128;
+        k_delayed<Real, D, RS, STAGE><<<grid1d(h->N, bs), bs, 0, h->stream>>>(Uin, (const Real*)h->U[0], Uout, g, h->sc);
+        h->launches += 1;
+      }
+    }
+  }
+
+  static void step(paraiso_hydro* h) {
+    stage<1>(h);
+    stage<2>(h);
+  }
+
+  static void cfl(paraiso_hydro* h) {
+    const Geom<Real> g = make_geom<Real>(h);
+    const int bs = 256;
+    int64_t blocks = (h->N + bs - 1) / bs;
+    if (blocks > 148 * 8) blocks = 148 * 8;
+    k_cfl<Real, D><<<(unsigned int)blocks, bs, 0, h->stream>>>((const Real*)h->U[0], g, h->sc);
+    h->launches += 1;
+  }
+
+  static void control(paraiso_hydro* h, int mode, double a, double b) {
+    k_control<Real><<<1, 1, 0, h->stream>>>(h->sc, make_geom<Real>(h), mode, a, b);
+    h->launches += 1;
+  }
+};
+
+template <class F>
+static void dispatch(paraiso_hydro* h, F&& f) {
+#define PH_CASE(REAL, DD)                                    \
+  if (h->riemann == RIEMANN_HLLC)                            \
+    f(Launch<REAL, DD, RIEMANN_HLLC>{});                     \
+  else                                                       \
+    f(Launch<REAL, DD, RIEMANN_HLL>{});
+  if (h->dtype == PARAISO_F32) {
+    if (h->dims == 1) { PH_CASE(float, 1) }
+    else if (h->dims == 2) { PH_CASE(float, 2) }
+    else { PH_CASE(float, 3) }
+  } else {
+    if (h->dims == 1) { PH_CASE(double, 1) }
+    else if (h->dims == 2) { PH_CASE(double, 2) }
+    else { PH_CASE(double, 3) }
+  }
+#undef PH_CASE
+}
+
+static int check_launch(paraiso_hydro* h) {
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(h, PARAISO_ECUDA, std::string("kernel launch: ") + cudaGetErrorString(e));
+  return PARAISO_OK;
+}
+
+static int options_key(const paraiso_hydro* h) {
+  int k = h->boundary | (h->riemann << 1) | (h->variant << 2);
+  k = k * 1031 + h->block[0];
+  k = k * 1031 + h->block[1];
+  k = k * 1031 + h->block[2];
+  k = k * 1031 + h->tile_depth;
+  k = k * 1031 + h->cells_per_thread;
+  return k & 0x7fffffff;
+}
+
+// ------------------------------------------------------------------------------------------------
+extern "C" {
+
+int paraiso_hydro_create(paraiso_hydro_t** out, int dims, const int64_t* n, const double* extent, double gamma,
+                         int dtype) {
+  if (!out || !n || !extent) return fail(nullptr, PARAISO_EINVAL, "create: null pointer");
+  if (dims < 1 || dims > 3) return fail(nullptr, PARAISO_EINVAL, "create: dims must be 1, 2 or 3");
+  if (dtype != PARAISO_F32 && dtype != PARAISO_F64) return fail(nullptr, PARAISO_EINVAL, "create: bad dtype");
+  if (!(gamma > 1.0) || !std::isfinite(gamma)) return fail(nullptr, PARAISO_EINVAL, "create: gamma must be > 1");
+  int64_t N = 1;
+  for (int a = 0; a < dims; ++a) {
+    if (n[a] < 4 || n[a] > (1ll << 30)) return fail(nullptr, PARAISO_EINVAL, "create: every n[a] must be >= 4");
+    if (!(extent[a] > 0.0) || !std::isfinite(extent[a])) return fail(nullptr, PARAISO_EINVAL, "create: extent must be > 0");
+    N *= n[a];
+    if (N > (1ll << 31) / 8) return fail(nullptr, PARAISO_EINVAL, "create: grid too large (nf*N must stay below 2^31)");
+  }
+  int ndev = 0;
+  cudaError_t e = cudaGetDeviceCount(&ndev);
+  if (e != cudaSuccess || ndev == 0)
+    return fail(nullptr, PARAISO_ECUDA,
+                std::string("create: no usable CUDA device (") + cudaGetErrorString(e) + "); there is no CPU fallback");
+  paraiso_hydro* h = new paraiso_hydro;
+  h->dims = dims;
+  h->dtype = dtype;
+  h->nf = dims + 2;
+  h->N = N;
+  h->gamma = gamma;
+  h->esize = dtype == PARAISO_F32 ? 4 : 8;
+  for (int a = 0; a < dims; ++a) {
+    h->n[a] = n[a];
+    h->extent[a] = extent[a];
+  }
+  const size_t bytes = size_t(h->nf) * N * h->esize;
+  for (int b = 0; b < 2; ++b) {
+    e = cudaMalloc(&h->U[b], bytes);
+    if (e != cudaSuccess) {
+      fail(nullptr, PARAISO_ENOMEM, std::string("create: cudaMalloc(state): ") + cudaGetErrorString(e));
+      paraiso_hydro_destroy(h);
+      return PARAISO_ENOMEM;
+    }
+  }
+  e = cudaMalloc((void**)&h->sc, sizeof(Scalars));
+  if (e == cudaSuccess) e = cudaMemset(h->sc, 0, sizeof(Scalars));
+  if (e != cudaSuccess) {
+    fail(nullptr, PARAISO_ENOMEM, std::string("create: scalars: ") + cudaGetErrorString(e));
+    paraiso_hydro_destroy(h);
+    return PARAISO_ENOMEM;
+  }
+  h->err = "no error";
+  *out = h;
+  return PARAISO_OK;
+}
+
+int paraiso_hydro_destroy(paraiso_hydro_t* h) {
+  if (!h) return PARAISO_OK;
+  cudaStreamSynchronize(h->stream);
+  drop_graph(h);
+  free_intermediates(h);
+  cudaFree(h->U[0]);
+  cudaFree(h->U[1]);
+  cudaFree(h->sc);
+  delete h;
+  return PARAISO_OK;
+}
+
+struct OptionRef {
+  int* field;
+  int64_t lo, hi;
+};
+
+static bool find_option(paraiso_hydro* h, const char* key, OptionRef* ref) {
+  struct Opt {
+    const char* key;
+    OptionRef ref;
+  };
+  const Opt opts[] = {{"boundary", {&h->boundary, 0, 1}},
+                      {"riemann", {&h->riemann, 0, 1}},
+                      {"variant", {&h->variant, 0, 3}},
+                      {"block_x", {&h->block[0], 0, 1024}},
+                      {"block_y", {&h->block[1], 0, 1024}},
+                      {"block_z", {&h->block[2], 0, 64}},
+                      {"tile_depth", {&h->tile_depth, 0, 1 << 20}},
+                      {"cells_per_thread", {&h->cells_per_thread, 0, 8}},
+                      {"graph", {&h->use_graph, 0, 1}}};
+  for (const Opt& o : opts)
+    if (!std::strcmp(key, o.key)) {
+      *ref = o.ref;
+      return true;
+    }
+  return false;
+}
+
+int paraiso_hydro_set_option(paraiso_hydro_t* h, const char* key, int64_t value) {
+  if (!h || !key) return fail(h, PARAISO_EINVAL, "set_option: null pointer");
+  OptionRef r;
+  if (!find_option(h, key, &r)) return fail(h, PARAISO_EINVAL, std::string("set_option: unknown key ") + key);
+  if (value < r.lo || value > r.hi) return fail(h, PARAISO_EINVAL, std::string("set_option: value out of range for ") + key);
+  *r.field = int(value);
+  return PARAISO_OK;
+}
+
+int paraiso_hydro_get_option(paraiso_hydro_t* h, const char* key, int64_t* value) {
+  if (!h || !key || !value) return fail(h, PARAISO_EINVAL, "get_option: null pointer");
+  OptionRef r;
+  if (!find_option(h, key, &r)) return fail(h, PARAISO_EINVAL, std::string("get_option: unknown key ") + key);
+  *value = *r.field;
+  return PARAISO_OK;
+}
+
+int paraiso_hydro_set_stream(paraiso_hydro_t* h, void* cuda_stream) {
+  if (!h) return fail(h, PARAISO_EINVAL, "set_stream: null handle");
+  CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+  h->stream = (cudaStream_t)cuda_stream;
+  drop_graph(h);
+  return PARAISO_OK;
+}
+
+int paraiso_hydro_set_state(paraiso_hydro_t* h, const void* U) {
+  if (!h || !U) return fail(h, PARAISO_EINVAL, "set_state: null pointer");
+  const size_t bytes = size_t(h->nf) * h->N * h->esize;
+  CUDA_TRY(h, cudaMemcpyAsync(h->U[0], U, bytes, cudaMemcpyDefault, h->stream));
+  dispatch(h, [&](auto L) {
+    L.control(h, CTRL_RESET, 0, 0);
+    L.cfl(h);
+  });
+  h->has_state = true;
+  return check_launch(h);
+}
+
+int paraiso_hydro_get_state(paraiso_hydro_t* h, void* U_out) {
+  if (!h || !U_out) return fail(h, PARAISO_EINVAL, "get_state: null pointer");
+  if (!h->has_state) return fail(h, PARAISO_ESTATE, "get_state: no state set");
+  const size_t bytes = size_t(h->nf) * h->N * h->esize;
+  CUDA_TRY(h, cudaMemcpyAsync(U_out, h->U[0], bytes, cudaMemcpyDefault, h->stream));
+  cudaPointerAttributes at;
+  cudaError_t e = cudaPointerGetAttributes(&at, U_out);
+  if (e != cudaSuccess || at.type == cudaMemoryTypeUnregistered || at.type == cudaMemoryTypeHost) {
+    cudaGetLastError();
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+  }
+  return PARAISO_OK;
+}
+
+int paraiso_hydro_cfl_dt(paraiso_hydro_t* h, double cfl, double* dt_out) {
+  if (!h || !dt_out) return fail(h, PARAISO_EINVAL, "cfl_dt: null pointer");
+  if (!(cfl > 0.0) || !std::isfinite(cfl)) return fail(h, PARAISO_EINVAL, "cfl_dt: cfl must be finite and > 0");
+  if (!h->has_state) return fail(h, PARAISO_ESTATE, "cfl_dt: no state set");
+  double S = 0;
+  CUDA_TRY(h, cudaMemcpyAsync(&S, &h->sc->S_last, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+  // same IEEE division, in the handle's precision, that the device finaliser performs
+  *dt_out = h->dtype == PARAISO_F32 ? double(float(cfl) / float(S)) : cfl / S;
+  return PARAISO_OK;
+}
+
+int paraiso_hydro_step(paraiso_hydro_t* h, double dt) {
+  if (!h) return fail(h, PARAISO_EINVAL, "step: null handle");
+  if (!h->has_state) return fail(h, PARAISO_ESTATE, "step: no state set");
+  if (!(dt > 0.0) || !std::isfinite(dt)) return fail(h, PARAISO_EINVAL, "step: dt must be finite and > 0");
+  int rc = ensure_intermediates(h);
+  if (rc) return rc;
+  dispatch(h, [&](auto L) {
+    L.control(h, CTRL_MANUAL_DT, dt, 0);
+    L.step(h);
+  });
+  return check_launch(h);
+}
+
+// Captures `nsteps` device-paced steps into a graph (kernels read dt and lambda from the scalar block, so the
+// same graph is valid for every step).
+static int capture_graph(paraiso_hydro* h, int nsteps) {
+  drop_graph(h);
+  cudaStream_t cap;
+  CUDA_TRY(h, cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
+  cudaStream_t user = h->stream;
+  h->stream = cap;
+  cudaGraph_t graph = nullptr;
+  cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
+  const int64_t before = h->launches;
+  if (e == cudaSuccess) {
+    dispatch(h, [&](auto L) {
+      for (int s = 0; s < nsteps; ++s) L.step(h);
+    });
+    e = cudaStreamEndCapture(cap, &graph);
+  }
+  h->launches = before;
+  h->stream = user;
+  if (e == cudaSuccess) e = cudaGraphInstantiate(&h->graph_exec, graph, 0);
+  if (graph) cudaGraphDestroy(graph);
+  cudaStreamDestroy(cap);
+  if (e != cudaSuccess) {
+    h->graph_exec = nullptr;
+    return fail(h, PARAISO_ECUDA, std::string("graph capture: ") + cudaGetErrorString(e));
+  }
+  h->graph_key = options_key(h);
+  h->graph_steps = nsteps;
+  return PARAISO_OK;
+}
+
+static int64_t launches_per_step(const paraiso_hydro* h) {
+  switch (h->variant) {
+    case VARIANT_MANIFEST_ALL: return 2 * (2 + 2 * h->dims);
+    case VARIANT_MANIFEST_FLUX: return 2 * (1 + h->dims);
+    default: return 2;
+  }
+}
+
+static int enqueue_steps(paraiso_hydro* h, int64_t nsteps) {
+  const int chunk = 8;  // steps per graph
+  int64_t left = nsteps;
+  if (h->use_graph && nsteps >= chunk) {
+    if (!h->graph_exec || h->graph_key != options_key(h) || h->graph_steps != chunk) {
+      int rc = capture_graph(h, chunk);
+      if (rc) return rc;
+    }
+    while (left >= chunk) {
+      CUDA_TRY(h, cudaGraphLaunch(h->graph_exec, h->stream));
+      h->launches += chunk * launches_per_step(h);
+      left -= chunk;
+    }
+  }
+  if (left > 0)
+    dispatch(h, [&](auto L) {
+      for (int64_t s = 0; s < left; ++s) L.step(h);
+    });
+  return check_launch(h);
+}
+
+int paraiso_hydro_run(paraiso_hydro_t* h, double cfl, int64_t nsteps, double t_end, int64_t* steps_done,
+                      double* t_out) {
+  if (!h) return fail(h, PARAISO_EINVAL, "run: null handle");
+  if (!h->has_state) return fail(h, PARAISO_ESTATE, "run: no state set");
+  if (!(cfl > 0.0) || !std::isfinite(cfl) || nsteps < 0) return fail(h, PARAISO_EINVAL, "run: bad cfl or nsteps");
+  int rc = ensure_intermediates(h);
+  if (rc) return rc;
+  dispatch(h, [&](auto L) { L.control(h, CTRL_BEGIN_RUN, cfl, t_end > 0.0 ? t_end : 0.0); });
+  if (!(t_end > 0.0)) {
+    rc = enqueue_steps(h, nsteps);
+    if (rc) return rc;
+    if (steps_done) *steps_done = nsteps;
+    return PARAISO_OK;
+  }
+  // t_end given: enqueue in chunks and look at the device clock between them; kernels of steps beyond
+  // t_end return immediately (Scalars::done).
+  struct {
+    double t;
+    long long steps;
+    int done;
+  } st = {0, 0, 0};
+  long long steps0 = 0;
+  CUDA_TRY(h, cudaMemcpyAsync(&steps0, &h->sc->steps, sizeof(long long), cudaMemcpyDeviceToHost, h->stream));
+  CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+  int64_t issued = 0;
+  while (issued < nsteps) {
+    const int64_t c = std::min<int64_t>(64, nsteps - issued);
+    rc = enqueue_steps(h, c);
+    if (rc) return rc;
+    issued += c;
+    CUDA_TRY(h, cudaMemcpyAsync(&st.t, &h->sc->t, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaMemcpyAsync(&st.steps, &h->sc->steps, sizeof(long long), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaMemcpyAsync(&st.done, &h->sc->done, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    if (st.done) break;
+  }
+  if (steps_done) *steps_done = st.steps - steps0;
+  if (t_out) *t_out = st.t;
+  return PARAISO_OK;
+}
+
+int paraiso_hydro_sync(paraiso_hydro_t* h) {
+  if (!h) return fail(h, PARAISO_EINVAL, "sync: null handle");
+  CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+  return PARAISO_OK;
+}
+
+int paraiso_hydro_time(paraiso_hydro_t* h, double* t_out, int64_t* steps_out) {
+  if (!h) return fail(h, PARAISO_EINVAL, "time: null handle");
+  double t = 0;
+  long long s = 0;
+  CUDA_TRY(h, cudaMemcpyAsync(&t, &h->sc->t, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  CUDA_TRY(h, cudaMemcpyAsync(&s, &h->sc->steps, sizeof(long long), cudaMemcpyDeviceToHost, h->stream));
+  CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+  if (t_out) *t_out = t;
+  if (steps_out) *steps_out = s;
+  return PARAISO_OK;
+}
+
+int paraiso_hydro_stats(paraiso_hydro_t* h, int64_t* nonfinite_cells) {
+  if (!h) return fail(h, PARAISO_EINVAL, "stats: null handle");
+  long long nf = 0;
+  CUDA_TRY(h, cudaMemcpyAsync(&nf, &h->sc->nonfinite, sizeof(long long), cudaMemcpyDeviceToHost, h->stream));
+  CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+  if (nonfinite_cells) *nonfinite_cells = nf;
+  if (nf > 0) return fail(h, PARAISO_ENONFINITE, "stats: non-finite or non-positive rho/p encountered");
+  return PARAISO_OK;
+}
+
+int paraiso_hydro_launch_count(paraiso_hydro_t* h, int64_t* launches) {
+  if (!h || !launches) return fail(h, PARAISO_EINVAL, "launch_count: null pointer");
+  *launches = h->launches;
+  return PARAISO_OK;
+}
+
+const char* paraiso_hydro_last_error(const paraiso_hydro_t* h) { return h ? h->err.c_str() : g_create_error.c_str(); }
+
+const char* paraiso_hydro_version(void) { return "paraiso_hydro 0.1 sm_100a"; }
+
+}  // extern "C"
