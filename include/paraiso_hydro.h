@@ -112,6 +112,15 @@ int paraiso_hydro_stats(paraiso_hydro_t *h, int64_t *nonfinite_cells);
 /* How many kernels the handle has launched since create (for bench.py's "gpu_launches"). */
 int paraiso_hydro_launch_count(paraiso_hydro_t *h, int64_t *launches);
 
+/* Per-stage device timing with CUDA events recorded on the handle's stream around the kernel(s) of every RK
+ * stage (for bench.py's roofline: the duration of the dominant kernel inside the timed region).
+ *   enable = 1 / 0  switch it on / off and reset the accumulators (blocks until the stream is idle); while on,
+ *                   run() launches plainly instead of replaying a graph
+ *   enable < 0      read: blocks until the recorded events have completed, then
+ *                   *total_ms = summed duration of the timed stages, *stage_launches = how many were timed.
+ * Either pointer may be NULL. */
+int paraiso_hydro_kernel_time(paraiso_hydro_t *h, int enable, double *total_ms, int64_t *stage_launches);
+
 /* Message for the last error on this handle (or the last create failure when h == NULL).  Never NULL. */
 const char *paraiso_hydro_last_error(const paraiso_hydro_t *h);
 

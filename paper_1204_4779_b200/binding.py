@@ -1,0 +1,225 @@
+"""ctypes binding of libparaiso_hydro.so — argument marshalling only (include/paraiso_hydro.h).
+
+Every function of the C ABI is exposed under the same name (`lib.paraiso_hydro_step`, ...) by
+`load_library()`; `ParaisoHydro` wraps one handle with methods of the same names minus the prefix.
+No step of the path runs here: state arrays go in and out as raw pointers (NumPy arrays = host
+pointers; torch CUDA tensors = device pointers, zero-copy), and PyTorch is used only for device
+memory and streams by callers who want them.
+
+There is no CPU fallback: if the library is not built, or no CUDA device is usable, this raises.
+"""
+import ctypes
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libparaiso_hydro.so")
+
+PARAISO_F32, PARAISO_F64 = 0, 1
+PARAISO_OK, PARAISO_EINVAL, PARAISO_ENOMEM, PARAISO_ECUDA, PARAISO_ESTATE, PARAISO_ENONFINITE = 0, -1, -2, -3, -4, -5
+
+BOUNDARY = {"periodic": 0, "outflow": 1}
+RIEMANN = {"hllc": 0, "hll": 1}
+VARIANT = {"fused": 0, "manifest_flux": 1, "manifest_all": 2, "delayed": 3}
+
+_vp, _i64, _dbl, _int = ctypes.c_void_p, ctypes.c_int64, ctypes.c_double, ctypes.c_int
+_pi64, _pdbl = ctypes.POINTER(_i64), ctypes.POINTER(_dbl)
+
+# name -> (restype, argtypes): one entry per symbol declared in include/paraiso_hydro.h
+SIGNATURES = {
+    "paraiso_hydro_create": (_int, [ctypes.POINTER(_vp), _int, _pi64, _pdbl, _dbl, _int]),
+    "paraiso_hydro_destroy": (_int, [_vp]),
+    "paraiso_hydro_set_option": (_int, [_vp, ctypes.c_char_p, _i64]),
+    "paraiso_hydro_get_option": (_int, [_vp, ctypes.c_char_p, _pi64]),
+    "paraiso_hydro_set_stream": (_int, [_vp, _vp]),
+    "paraiso_hydro_set_state": (_int, [_vp, _vp]),
+    "paraiso_hydro_get_state": (_int, [_vp, _vp]),
+    "paraiso_hydro_cfl_dt": (_int, [_vp, _dbl, _pdbl]),
+    "paraiso_hydro_step": (_int, [_vp, _dbl]),
+    "paraiso_hydro_run": (_int, [_vp, _dbl, _i64, _dbl, _pi64, _pdbl]),
+    "paraiso_hydro_sync": (_int, [_vp]),
+    "paraiso_hydro_time": (_int, [_vp, _pdbl, _pi64]),
+    "paraiso_hydro_stats": (_int, [_vp, _pi64]),
+    "paraiso_hydro_launch_count": (_int, [_vp, _pi64]),
+    "paraiso_hydro_kernel_time": (_int, [_vp, _int, _pdbl, _pi64]),
+    "paraiso_hydro_last_error": (ctypes.c_char_p, [_vp]),
+    "paraiso_hydro_version": (ctypes.c_char_p, []),
+}
+
+_LIB = None
+
+
+class ParaisoError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"paraiso_hydro error {code}: {msg}")
+        self.code = code
+
+
+def load_library(path=None):
+    """dlopen the C-ABI library and declare every prototype.  Raises if it has not been built
+    (`python -m paper_1204_4779_b200.build`): the product path never falls back to anything else."""
+    global _LIB
+    if _LIB is not None and path is None:
+        return _LIB
+    p = path or LIB_PATH
+    if not os.path.exists(p):
+        raise ParaisoError(PARAISO_ECUDA, f"{p} not built; run `python -m paper_1204_4779_b200.build` "
+                                          "(there is no CPU fallback)")
+    lib = ctypes.CDLL(p)
+    for name, (res, args) in SIGNATURES.items():
+        fn = getattr(lib, name)  # AttributeError if a declared symbol is not exported
+        fn.restype = res
+        fn.argtypes = args
+    if path is None:
+        _LIB = lib
+    return lib
+
+
+def _pointer(a):
+    """Raw address of a NumPy array (host) or a torch tensor (host or device).  The caller keeps it alive."""
+    if isinstance(a, np.ndarray):
+        if not a.flags["C_CONTIGUOUS"]:
+            raise ValueError("state array must be C-contiguous")
+        return a.ctypes.data, a.dtype, a.size
+    if hasattr(a, "data_ptr"):  # torch.Tensor
+        if not a.is_contiguous():
+            raise ValueError("state tensor must be contiguous")
+        import torch
+
+        dt = {torch.float32: np.dtype(np.float32), torch.float64: np.dtype(np.float64)}[a.dtype]
+        return a.data_ptr(), dt, a.numel()
+    raise TypeError(f"unsupported state container {type(a)}")
+
+
+class ParaisoHydro:
+    """One solver handle.  n is (nx[, ny[, nz]]) — x first; state arrays are (nf, [nz,] [ny,] nx)."""
+
+    def __init__(self, n, extent, gamma, dtype, boundary="periodic", riemann="hllc", variant=None, stream=None,
+                 **options):
+        self._lib = load_library()
+        self._h = _vp()
+        self.n = tuple(int(v) for v in n)
+        self.dims = len(self.n)
+        self.nf = self.dims + 2
+        self.dtype = np.dtype(dtype)
+        self.shape = (self.nf,) + tuple(reversed(self.n))
+        if self.dtype not in (np.dtype(np.float32), np.dtype(np.float64)):
+            raise ValueError("dtype must be float32 or float64")
+        narr = (_i64 * self.dims)(*self.n)
+        earr = (_dbl * self.dims)(*[float(e) for e in extent])
+        rc = self._lib.paraiso_hydro_create(ctypes.byref(self._h), self.dims, narr, earr, float(gamma),
+                                            PARAISO_F32 if self.dtype == np.float32 else PARAISO_F64)
+        if rc != PARAISO_OK:
+            msg = self._lib.paraiso_hydro_last_error(None).decode()
+            self._h = _vp()
+            raise ParaisoError(rc, msg)
+        self.set_option("boundary", BOUNDARY[boundary] if isinstance(boundary, str) else boundary)
+        self.set_option("riemann", RIEMANN[riemann] if isinstance(riemann, str) else riemann)
+        if variant is not None:
+            self.set_option("variant", VARIANT[variant] if isinstance(variant, str) else variant)
+        for k, v in options.items():
+            self.set_option(k, v)
+        if stream is not None:
+            self.set_stream(stream)
+
+    # -- plumbing
+    def _check(self, rc):
+        if rc != PARAISO_OK:
+            raise ParaisoError(rc, self._lib.paraiso_hydro_last_error(self._h).decode())
+
+    def _state_ptr(self, a):
+        ptr, dt, size = _pointer(a)
+        if dt != self.dtype:
+            raise ValueError(f"state dtype {dt} does not match the handle's {self.dtype}")
+        if size != int(np.prod(self.shape)):
+            raise ValueError(f"state has {size} elements, expected {self.shape}")
+        return ptr
+
+    # -- the C ABI, one method per entry point
+    def set_option(self, key, value):
+        self._check(self._lib.paraiso_hydro_set_option(self._h, key.encode(), int(value)))
+
+    def get_option(self, key):
+        v = _i64(0)
+        self._check(self._lib.paraiso_hydro_get_option(self._h, key.encode(), ctypes.byref(v)))
+        return v.value
+
+    def set_stream(self, stream):
+        """stream: a raw cudaStream_t integer or a torch.cuda.Stream."""
+        s = getattr(stream, "cuda_stream", stream)
+        self._check(self._lib.paraiso_hydro_set_stream(self._h, _vp(int(s) if s else 0)))
+
+    def set_state(self, U):
+        self._check(self._lib.paraiso_hydro_set_state(self._h, _vp(self._state_ptr(U))))
+
+    def get_state(self, out=None):
+        if out is None:
+            out = np.empty(self.shape, self.dtype)
+        self._check(self._lib.paraiso_hydro_get_state(self._h, _vp(self._state_ptr(out))))
+        return out
+
+    def cfl_dt(self, cfl):
+        dt = _dbl(0)
+        self._check(self._lib.paraiso_hydro_cfl_dt(self._h, float(cfl), ctypes.byref(dt)))
+        return dt.value
+
+    def step(self, dt):
+        self._check(self._lib.paraiso_hydro_step(self._h, float(dt)))
+
+    def run(self, cfl, nsteps, t_end=0.0):
+        k, t = _i64(0), _dbl(0)
+        self._check(self._lib.paraiso_hydro_run(self._h, float(cfl), int(nsteps), float(t_end), ctypes.byref(k),
+                                                ctypes.byref(t)))
+        return k.value, t.value
+
+    def sync(self):
+        self._check(self._lib.paraiso_hydro_sync(self._h))
+
+    def time(self):
+        t, k = _dbl(0), _i64(0)
+        self._check(self._lib.paraiso_hydro_time(self._h, ctypes.byref(t), ctypes.byref(k)))
+        return t.value, k.value
+
+    def stats(self):
+        """Number of cell updates that produced a non-finite or non-positive rho / p (0 = healthy)."""
+        k = _i64(0)
+        rc = self._lib.paraiso_hydro_stats(self._h, ctypes.byref(k))
+        if rc not in (PARAISO_OK, PARAISO_ENONFINITE):
+            self._check(rc)
+        return k.value
+
+    def launch_count(self):
+        k = _i64(0)
+        self._check(self._lib.paraiso_hydro_launch_count(self._h, ctypes.byref(k)))
+        return k.value
+
+    def kernel_time(self, enable=None):
+        """enable=1/0 switches per-stage CUDA-event timing on the handle's stream on or off (and resets
+        the accumulators); enable=None reads (total stage-kernel milliseconds, stage launches timed)."""
+        ms, k = _dbl(0), _i64(0)
+        self._check(self._lib.paraiso_hydro_kernel_time(self._h, -1 if enable is None else int(enable),
+                                                        ctypes.byref(ms), ctypes.byref(k)))
+        return ms.value, k.value
+
+    def version(self):
+        return self._lib.paraiso_hydro_version().decode()
+
+    def destroy(self):
+        if getattr(self, "_h", None) and self._h.value:
+            self._lib.paraiso_hydro_destroy(self._h)
+            self._h = _vp()
+
+    close = destroy
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.destroy()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass

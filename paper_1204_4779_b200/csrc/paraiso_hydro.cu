@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstring>
 #include <string>
+#include <vector>
 
 #include "hydro_kernels_basic.cuh"
 #include "hydro_kernels_fused.cuh"
@@ -37,6 +38,13 @@ struct paraiso_hydro {
   cudaStream_t stream = nullptr;
   bool has_state = false;
   int64_t launches = 0;
+
+  // optional per-stage CUDA-event timing on the handle's stream (paraiso_hydro_kernel_time)
+  bool timing = false;
+  std::vector<cudaEvent_t> ev;  // pairs (before, after) of the stage launches not yet read back
+  size_t ev_used = 0;
+  double timed_ms = 0;
+  int64_t timed_count = 0;
 
   cudaGraphExec_t graph_exec = nullptr;
   int graph_key = -1;  // option fingerprint the graph was captured with
@@ -89,6 +97,35 @@ static void free_intermediates(paraiso_hydro* h) {
     cudaFree(h->Fb[a]);
     h->LO[a] = h->HI[a] = h->F[a] = h->Fb[a] = nullptr;
   }
+}
+
+// Sum up and recycle the recorded event pairs (blocks until the last one has completed).
+static void drain_events(paraiso_hydro* h) {
+  if (h->ev_used == 0) return;
+  cudaEventSynchronize(h->ev[h->ev_used - 1]);
+  for (size_t i = 0; i + 1 < h->ev_used; i += 2) {
+    float ms = 0;
+    if (cudaEventElapsedTime(&ms, h->ev[i], h->ev[i + 1]) == cudaSuccess) {
+      h->timed_ms += ms;
+      h->timed_count += 1;
+    }
+  }
+  h->ev_used = 0;
+}
+
+static cudaEvent_t next_event(paraiso_hydro* h) {
+  if (h->ev_used == h->ev.size()) {
+    if (h->ev.size() >= 4096) {
+      drain_events(h);
+    } else {
+      cudaEvent_t e = nullptr;
+      cudaEventCreate(&e);
+      h->ev.push_back(e);
+    }
+  }
+  cudaEvent_t e = h->ev[h->ev_used++];
+  cudaEventRecord(e, h->stream);
+  return e;
 }
 
 static void drop_graph(paraiso_hydro* h) {
@@ -155,6 +192,13 @@ struct Launch {
     const Geom<Real> g = make_geom<Real>(h);
     const Real* Uin = (const Real*)(STAGE == 1 ? h->U[0] : h->U[1]);
     Real* Uout = (Real*)(STAGE == 1 ? h->U[1] : h->U[0]);
+    if (h->timing) next_event(h);
+    stage_kernels<STAGE>(h, g, Uin, Uout);
+    if (h->timing) next_event(h);
+  }
+
+  template <int STAGE>
+  static void stage_kernels(paraiso_hydro* h, const Geom<Real>& g, const Real* Uin, Real* Uout) {
     switch (h->variant) {
       case VARIANT_MANIFEST_ALL: {
         const int bs = 256;
@@ -301,6 +345,7 @@ int paraiso_hydro_destroy(paraiso_hydro_t* h) {
   cudaStreamSynchronize(h->stream);
   drop_graph(h);
   free_intermediates(h);
+  for (cudaEvent_t e : h->ev) cudaEventDestroy(e);
   cudaFree(h->U[0]);
   cudaFree(h->U[1]);
   cudaFree(h->sc);
@@ -453,7 +498,7 @@ static int64_t launches_per_step(const paraiso_hydro* h) {
 static int enqueue_steps(paraiso_hydro* h, int64_t nsteps) {
   const int chunk = 8;  // steps per graph
   int64_t left = nsteps;
-  if (h->use_graph && nsteps >= chunk) {
+  if (h->use_graph && !h->timing && nsteps >= chunk) {
     if (!h->graph_exec || h->graph_key != options_key(h) || h->graph_steps != chunk) {
       int rc = capture_graph(h, chunk);
       if (rc) return rc;
@@ -543,6 +588,22 @@ int paraiso_hydro_stats(paraiso_hydro_t* h, int64_t* nonfinite_cells) {
 int paraiso_hydro_launch_count(paraiso_hydro_t* h, int64_t* launches) {
   if (!h || !launches) return fail(h, PARAISO_EINVAL, "launch_count: null pointer");
   *launches = h->launches;
+  return PARAISO_OK;
+}
+
+int paraiso_hydro_kernel_time(paraiso_hydro_t* h, int enable, double* total_ms, int64_t* stage_launches) {
+  if (!h) return fail(h, PARAISO_EINVAL, "kernel_time: null handle");
+  if (enable >= 0) {
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    h->ev_used = 0;
+    h->timed_ms = 0;
+    h->timed_count = 0;
+    h->timing = enable != 0;
+  } else {
+    drain_events(h);
+  }
+  if (total_ms) *total_ms = h->timed_ms;
+  if (stage_launches) *stage_launches = h->timed_count;
   return PARAISO_OK;
 }
 
