@@ -1,0 +1,378 @@
+"""bench.py — Gcell-updates/s per full RK2 step of the Euler hot path (BASELINE.json metric) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--variant fused] [--riemann hllc]
+                    [--impl reference] [--no-sweep] [--no-cpu]
+
+A "step" = one full RK2 step (both stages a1-a5 + the CFL reduction a0, dt read on the device from the
+previous step's fused reduction) of one synthetic workload.  Default workload = BASELINE
+config 4 (3-D blast 512^3 fp32, 2.7 GB per state buffer: larger than L2, no flush needed); the other configs
+are added to the same JSON line under "all_configs" (short runs; config 1 is L2-resident, said so there).
+
+  value     cells * steps / device time (CUDA events on the handle's stream, max over ranks), state resident in HBM
+  e2e       same metric through the C ABI with HOST (pinned) buffers: set_state(host) + cfl_dt + step +
+            get_state(host) every step, copies inside the timed region
+  roofline  dominant kernel = the RK stage kernel; algorithmic bytes per launch = 2*nf*w*N (state read once,
+            written once per stage; north_star's definition) / average stage duration measured
+            with CUDA events around every stage launch inside the timed region; peak = MEASURED_PEAKS.json
+  cpu_baseline  the oracle as it stands, single-threaded and OpenMP, on a bounded sample of the same workload
+
+N > 1: replicas only: every rank advances its own copy of the workload, no data-path collective;
+value = all ranks' cell updates / max-over-ranks time, "scaling": "weak".
+--impl reference: the oracle (oracle/, OpenMP build) timed on the host cores; rank 0 only.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "Gcell-updates/s per RK2 step"
+UNIT = "Gcell/s"
+DEFAULT_STEPS = {0: 279, 1: 100, 2: 50, 3: 50, 4: 20}
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            d = json.load(open(p))
+            return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md clocks line)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc, self.thread = index, [], None, None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            return self
+        self.thread = threading.Thread(target=self._read, daemon=True)
+        self.thread.start()
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), [c.strip() for c in line.split(",")]))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        rows = [r for t, r in self.rows if t0 <= t <= t1 + 0.1] or [r for _, r in self.rows[-3:]]
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in rows:
+            try:
+                sm.append(float(r[0]))
+                mx.append(float(r[1]))
+                pw.append(float(r[2]))
+            except (ValueError, IndexError):
+                continue
+            for name, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def algorithmic_bytes_per_cell_step(w):
+    """north_star roofline (a): state read and written once per stage, halo excluded = 4*nf*w bytes per cell-step."""
+    return 4 * w.nf * w.dtype.itemsize
+
+
+def make_workload(cfg):
+    from paper_1204_4779_b200 import inputs
+
+    return inputs.baseline_config(cfg)
+
+
+def centred_sample(w, edge):
+    """A centred sub-box (edge cells per axis, at most the grid) of the workload's own initial state, as a
+    periodic problem of the same mesh size: the bounded sample the oracle is timed on."""
+    from paper_1204_4779_b200 import inputs
+
+    sl = [slice(None)]
+    n = []
+    for a in reversed(range(w.dims)):  # array axes are [f][z][y][x]
+        m = min(edge, w.n[a])
+        lo = (w.n[a] - m) // 2
+        sl.append(slice(lo, lo + m))
+        n.append(m)
+    n = tuple(reversed(n))
+    U = np.ascontiguousarray(w.U[tuple(sl)])
+    ext = tuple(w.extent[a] * n[a] / w.n[a] for a in range(w.dims))
+    return inputs.Workload(w.name + "_sample" + "x".join(map(str, n)), n, ext, w.gamma, w.dtype, "periodic", w.cfl, 0, 0.0, U)
+
+
+def oracle_rate(w, steps, warmup, threads):
+    """Gcell/s of the oracle (oracle/euler_oracle.cpp as it stands) on workload w; returns (rate, seconds, cores)."""
+    import oracle
+
+    o = oracle.Oracle(w.n, w.extent, w.gamma, w.dtype, w.boundary, "hllc", threads)
+    o.set_state(w.U)
+    for _ in range(warmup):
+        o.step(o.cfl_dt(w.cfl))
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        o.step(o.cfl_dt(w.cfl))
+    dt = time.perf_counter() - t0
+    o.close()
+    cores = oracle.num_threads("omp") if threads == "omp" else 1
+    return w.cells * steps / dt / 1e9, dt, cores
+
+
+def cpu_baseline(w):
+    edge = {1: 1 << 20, 2: 1536, 3: 144}[w.dims]
+    s = centred_sample(w, edge)
+    r1, t1, _ = oracle_rate(s, 1, 1, "serial")
+    steps = max(2, int(8.0 / max(t1 / 8, 1e-3) / 8))  # ~8 s of OpenMP work if it scales, capped below
+    steps = min(steps, 12)
+    rn, tn, cores = oracle_rate(s, steps, 1, "omp")
+    return {"value": rn, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"centred {'x'.join(map(str, s.n))} sub-box of the workload's initial state, periodic, "
+                      f"{steps} RK2 steps (OpenMP build of oracle/euler_oracle.cpp, bit-identical to serial)",
+            "serial_value": r1, "serial_cores": 1, "seconds": t1 * 2 + tn}
+
+
+def reference_arm(args):
+    """--impl reference: the oracle timed on the host cores, same metric / config keys; rank 0 only."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    w = make_workload(args.config)
+    edge = {1: 1 << 20, 2: 1024, 3: 128}[w.dims]
+    s = centred_sample(w, edge)
+    rate, secs, cores = oracle_rate(s, args.steps, args.warmup, "omp")
+    sample = (f"each step = one oracle RK2 step (+ CFL reduction) on the centred {'x'.join(map(str, s.n))} sub-box of "
+              f"config {args.config}'s initial state, periodic")
+    line = {"impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": secs / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32" if w.dtype == np.float32 else "f64", "data": "synthetic",
+            "config": {"workload": f"BASELINE config {args.config}: {w.name}", "grid": list(w.n), "riemann": "hllc",
+                       "sample": sample},
+            "cpu_baseline": {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": rate, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def device_run(binding, torch, w, steps, warmup, variant, riemann, per_stage, options=None):
+    """K device-paced steps with the state resident in HBM; returns dict(ms, stage_ms, stage_launches, launches)."""
+    s = torch.cuda.Stream()
+    with binding.ParaisoHydro(w.n, w.extent, w.gamma, w.dtype, w.boundary, riemann, variant, stream=s,
+                              **(options or {})) as h:
+        dev = torch.from_numpy(w.U).cuda()
+        h.set_state(dev)
+        del dev
+        h.run(w.cfl, warmup)
+        h.sync()
+        if per_stage:
+            h.kernel_time(1)
+        l0 = h.launch_count()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record(s)
+        h.run(w.cfl, steps)
+        e1.record(s)
+        e1.synchronize()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1)
+        stage_ms, stage_n = h.kernel_time() if per_stage else (ms, 2 * steps)
+        if per_stage:
+            h.kernel_time(0)
+        launches = h.launch_count() - l0
+        bad = h.stats()
+        t, k = h.time()
+        if bad or k != steps + warmup:
+            raise RuntimeError(f"bench run unhealthy: nonfinite={bad} steps={k}")
+    return {"ms": ms, "stage_ms": stage_ms, "stage_launches": stage_n, "launches": launches, "t": t}
+
+
+def e2e_run(binding, torch, w, steps, warmup, variant, riemann):
+    """The same metric through the C ABI with HOST buffers: every step copies the state host -> device
+    (set_state from pinned memory), computes dt (cfl_dt), advances one RK2 step and copies the result back."""
+    src = torch.from_numpy(w.U).pin_memory()
+    dst = torch.empty_like(src).pin_memory()
+    s = torch.cuda.Stream()
+    with binding.ParaisoHydro(w.n, w.extent, w.gamma, w.dtype, w.boundary, riemann, variant, stream=s) as h:
+        def one(inp, out):
+            h.set_state(inp)
+            h.step(h.cfl_dt(w.cfl))
+            h.get_state(out)
+
+        one(src, dst)
+        for _ in range(max(0, warmup - 1)):
+            one(dst, dst)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        e0.record(s)
+        for _ in range(steps):
+            one(dst, dst)
+        e1.record(s)
+        e1.synchronize()
+        wall = time.perf_counter() - t0
+        ms = max(e0.elapsed_time(e1), wall * 1e3)  # host-blocking calls are part of the end-to-end time
+        assert bool(torch.isfinite(dst).all())
+    nbytes = w.U.nbytes
+    return {"value": w.cells * steps / (ms * 1e-3) / 1e9, "unit": UNIT, "h2d_bytes_per_step": nbytes,
+            "d2h_bytes_per_step": nbytes, "ms_per_step": ms / steps, "steps": steps}
+
+
+def roofline_of(w, r, peak, peak_src, traffic=None):
+    nbytes = 2 * w.nf * w.dtype.itemsize * w.cells  # one stage launch: read the state once, write it once
+    avg_ms = r["stage_ms"] / max(1, r["stage_launches"])
+    achieved = nbytes / (avg_ms * 1e-3) / 1e9
+    return {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+            "traffic": traffic, "kernel": "RK stage kernel(s) (a1-a5 [+a0 in stage 2])",
+            "algorithmic_bytes_per_launch": nbytes, "avg_launch_ms": avg_ms, "peak_source": peak_src}
+
+
+def ncu_traffic(cfg, variant):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, copied by hand from the
+    committed ncu --set full capture (profiles/traffic.json names the capture); None if not captured."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if not os.path.exists(p):
+        return None
+    try:
+        return json.load(open(p)).get(f"config{cfg}:{variant}")
+    except Exception:
+        return None
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--variant", default="fused")
+    ap.add_argument("--riemann", default="hllc")
+    ap.add_argument("--impl", default="b200")
+    ap.add_argument("--no-sweep", action="store_true", help="skip the short runs of the other configs / variants")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--opt", action="append", default=[], help="key=value launch-shape option (block_x, ...)")
+    args = ap.parse_args()
+    if args.steps is None:
+        args.steps = DEFAULT_STEPS[args.config]
+    args.warmup = max(args.warmup, 0)
+    if args.impl == "reference":
+        return reference_arm(args)
+
+    import torch
+    import torch.distributed as dist
+
+    from paper_1204_4779_b200 import binding
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    binding.load_library()
+    options = {k: int(v) for k, v in (o.split("=") for o in args.opt)}
+
+    w = make_workload(args.config)
+    big = w.cells >= (1 << 22)  # per-stage events only where a stage is >> an event record
+    peak, peak_src = measured_peaks()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    barrier()
+    sampler = ClockSampler(local).start() if rank == 0 else None
+    t0 = time.time()
+    r = device_run(binding, torch, w, args.steps, args.warmup, args.variant, args.riemann, big, options)
+    t1 = time.time()
+    barrier()
+    clocks = sampler.stop(t0, t1) if sampler else None
+    ms = r["ms"]
+    if world > 1:
+        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = w.cells * args.steps * world / (ms * 1e-3) / 1e9
+
+    e2e = None
+    if not args.no_e2e:
+        e = e2e_run(binding, torch, w, min(args.steps, 5), min(args.warmup, 2), args.variant, args.riemann)
+        ev = e["value"] * world
+        if world > 1:
+            t = torch.tensor([e["ms_per_step"]], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ev = w.cells * world / (float(t.item()) * 1e-3) / 1e9
+        e2e = dict(e, value=ev, h2d_bytes_per_step=e["h2d_bytes_per_step"] * world,
+                   d2h_bytes_per_step=e["d2h_bytes_per_step"] * world)
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32" if w.dtype == np.float32 else "f64", "data": "synthetic",
+            "config": {"workload": f"BASELINE config {args.config}: {w.name}", "grid": list(w.n), "fields": w.nf,
+                       "gamma": w.gamma, "cfl": w.cfl, "boundary": w.boundary, "riemann": args.riemann,
+                       "variant": args.variant, "options": options, "parallelism": "replicas" if world > 1 else "1gpu",
+                       "l2": "state buffers (2 x %.0f MB) exceed the 126 MB L2; no flush needed" % (w.U.nbytes / 1e6)
+                       if 2 * w.U.nbytes > 126e6 else "L2-RESIDENT workload (2 x %.1f MB): not an HBM number" % (w.U.nbytes / 1e6)},
+            "roofline": roofline_of(w, r, peak, peak_src, ncu_traffic(args.config, args.variant)),
+            "e2e": e2e, "gpu_launches": r["launches"], "clocks": clocks}
+
+    if rank == 0 and not args.no_sweep:
+        line["all_configs"] = sweep(binding, torch, args, peak, peak_src)
+    if rank == 0 and not args.no_cpu:
+        line["cpu_baseline"] = cpu_baseline(w)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+
+
+def sweep(binding, torch, args, peak, peak_src):
+    """Short runs of every BASELINE config with every kernel variant (the Manifest <-> Delayed axis), same protocol."""
+    out = []
+    for cfg in (0, 1, 2, 3, 4):
+        w = make_workload(cfg)
+        big = w.cells >= (1 << 22)
+        steps = min(DEFAULT_STEPS[cfg], 100 if not big else 10)
+        for variant in ("fused", "manifest_flux", "manifest_all", "delayed"):
+            try:
+                r = device_run(binding, torch, w, steps, 3, variant, args.riemann, big)
+            except Exception as ex:  # e.g. out of memory for manifest_all
+                out.append({"config": cfg, "variant": variant, "error": str(ex)[:120]})
+                continue
+            rl = roofline_of(w, r, peak, peak_src)
+            out.append({"config": cfg, "workload": w.name, "variant": variant, "steps": steps,
+                        "value": w.cells * steps / (r["ms"] * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": r["ms"] / steps,
+                        "hbm_frac": rl["frac"], "algorithmic_gbs": rl["achieved"], "launches": r["launches"]})
+        del w
+    return out
+
+
+if __name__ == "__main__":
+    main()

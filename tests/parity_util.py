@@ -1,0 +1,31 @@
+"""Helpers shared by the GPU parity tests: the error metric of DESIGN.md R17 and an oracle runner."""
+import numpy as np
+
+# north_star tolerances: (one step, 100 steps, dt)
+TOL = {np.dtype(np.float64): (1e-12, 1e-9, 1e-13), np.dtype(np.float32): (1e-5, 1e-3, 1e-6)}
+
+
+def field_errors(got, ref):
+    """err_f = max_i |got_f - ref_f| / max_i |ref_f| per conserved field (R17).  The momentum
+    components share the scale max_b max_i |m_b|: a component that is ~0 everywhere has no scale of its own."""
+    nf = ref.shape[0]
+    g = got.reshape(nf, -1).astype(np.float64)
+    r = ref.reshape(nf, -1).astype(np.float64)
+    scale = np.abs(r).max(axis=1)
+    mom = scale[1:nf - 1].max()
+    scale[1:nf - 1] = np.maximum(scale[1:nf - 1], mom)
+    scale = np.where(scale > 0, scale, 1.0)
+    return np.abs(g - r).max(axis=1) / scale
+
+
+def oracle_steps(oracle_mod, w, nsteps, riemann="hllc", threads="omp", boundary=None, cfl=None):
+    """Run the oracle nsteps steps with its own CFL dt; returns (state, [dt_k])."""
+    o = oracle_mod.Oracle(w.n, w.extent, w.gamma, w.dtype, boundary or w.boundary, riemann, threads)
+    o.set_state(w.U)
+    dts = []
+    for _ in range(nsteps):
+        dts.append(o.cfl_dt(cfl or w.cfl))
+        o.step(dts[-1])
+    out = o.get_state()
+    o.close()
+    return out, dts

@@ -1,0 +1,208 @@
+"""GPU parity: the CUDA path, called through the C ABI, against the CPU oracle on the same seeded inputs.
+
+Element-by-element comparison with the metric of DESIGN.md R17 and north_star's tolerances
+(fp64: 1e-12 after one step, 1e-9 after 100, dt 1e-13; fp32: 1e-5, 1e-3, 1e-6).  Grids are small
+enough for the oracle to finish in seconds but span several thread blocks / tiles with ragged tails.
+Full-size BASELINE configs: tests/test_gpu_configs.py.
+"""
+import numpy as np
+import pytest
+
+from parity_util import TOL, field_errors, oracle_steps
+from paper_1204_4779_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+VARIANTS = ["fused", "manifest_flux", "manifest_all", "delayed"]
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1204_4779_b200 import binding
+
+    binding.load_library()  # raises if the extension is missing: no fallback
+    return binding
+
+
+def gpu_steps(binding, w, nsteps, variant, riemann="hllc", boundary=None, cfl=None, **opts):
+    import torch
+
+    with binding.ParaisoHydro(w.n, w.extent, w.gamma, w.dtype, boundary or w.boundary, riemann, variant, **opts) as h:
+        h.set_state(torch.from_numpy(w.U).cuda())
+        dts = []
+        for _ in range(nsteps):
+            dts.append(h.cfl_dt(cfl or w.cfl))
+            h.step(dts[-1])
+        got = h.get_state()
+        assert h.stats() == 0
+        assert h.time()[1] == nsteps
+    return got, dts
+
+
+# ragged shapes: not multiples of any block/tile edge, several tiles per axis
+SHAPES = {1: (1000,), 2: (203, 77), 3: (45, 38, 27)}
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("riemann", ["hllc", "hll"])
+@pytest.mark.parametrize("boundary", ["periodic", "outflow"])
+@pytest.mark.parametrize("dims", [1, 2, 3])
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_one_and_three_steps_match_oracle(gpu, oracle_mod, variant, dims, boundary, riemann, dtype):
+    w = inputs.random_smooth(SHAPES[dims], dtype, seed=10 + dims, boundary=boundary)
+    tol1, _, told = TOL[np.dtype(dtype)]
+    for nsteps in (1, 3):
+        ref, rdt = oracle_steps(oracle_mod, w, nsteps, riemann)
+        got, gdt = gpu_steps(gpu, w, nsteps, variant, riemann)
+        for a, b in zip(gdt, rdt):
+            assert abs(a - b) <= told * b, (a, b)
+        err = field_errors(got, ref)
+        assert np.all(err <= tol1 * nsteps), (variant, nsteps, err)
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("dims", [1, 2, 3])
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_hundred_steps_match_oracle(gpu, oracle_mod, variant, dims, dtype):
+    n = {1: (517,), 2: (130, 61), 3: (37, 30, 21)}[dims]
+    w = inputs.random_smooth(n, dtype, seed=20 + dims)
+    _, tol100, told = TOL[np.dtype(dtype)]
+    ref, rdt = oracle_steps(oracle_mod, w, 100)
+    got, gdt = gpu_steps(gpu, w, 100, variant)
+    assert abs(gdt[-1] - rdt[-1]) <= max(told, tol100 * 1e-1) * rdt[-1]
+    err = field_errors(got, ref)
+    assert np.all(err <= tol100), (variant, err)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("n", [(4,), (5,), (4, 4), (4, 7), (4, 4, 4), (6, 4, 5)])
+def test_minimum_size_grids(gpu, oracle_mod, variant, n):
+    """n_a = 4 is the smallest legal periodic axis (stencil reach 2): every halo wraps onto the tile itself."""
+    for boundary in ("periodic", "outflow"):
+        w = inputs.random_smooth(n, np.float64, seed=3, boundary=boundary)
+        ref, _ = oracle_steps(oracle_mod, w, 2)
+        got, _ = gpu_steps(gpu, w, 2, variant)
+        assert np.all(field_errors(got, ref) <= 2e-12), (n, boundary)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_uniform_state_is_bitwise_fixed_on_the_gpu(gpu, variant, dtype):
+    import torch
+
+    for n in [(64,), (40, 33), (20, 18, 17)]:
+        dims = len(n)
+        shape = tuple(reversed(n))
+        U = inputs.conserved_from_primitive(np.full(shape, 1.3), [np.full(shape, v) for v in (0.37, -1.9, 2.3)[:dims]],
+                                            np.full(shape, 0.7), 1.4).astype(dtype)
+        with gpu.ParaisoHydro(n, [1.0] * dims, 1.4, dtype, "periodic", "hllc", variant) as h:
+            h.set_state(np.ascontiguousarray(U))
+            for _ in range(4):
+                h.step(h.cfl_dt(0.4))
+            assert np.array_equal(h.get_state(), U)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_device_paced_run_matches_oracle_run(gpu, oracle_mod, variant):
+    """run(): dt from the device-resident CFL reduction, CUDA-graph replay; 21 steps = 2 graphs of 8 + 5 plain."""
+    import torch
+
+    for w in (inputs.kelvin_helmholtz(96, 72, np.float64, seed=5), inputs.blast(dtype=np.float32, seed=6, shape=(33, 29, 31))):
+        o = oracle_mod.Oracle(w.n, w.extent, w.gamma, w.dtype, w.boundary, "hllc", "omp")
+        o.set_state(w.U)
+        k, t = o.run(w.cfl, 21)
+        ref = o.get_state()
+        with gpu.ParaisoHydro(w.n, w.extent, w.gamma, w.dtype, w.boundary, "hllc", variant) as h:
+            h.set_state(torch.from_numpy(w.U).cuda())
+            h.run(w.cfl, 21)
+            tg, kg = h.time()
+            got = h.get_state()
+        assert kg == k == 21
+        _, tol100, _ = TOL[w.dtype]
+        assert abs(tg - t) <= 1e-6 * t if w.dtype == np.float32 else abs(tg - t) <= 1e-12 * t
+        assert np.all(field_errors(got, ref) <= tol100)
+
+
+@pytest.mark.parametrize("riemann", ["hll", "hllc"])
+def test_config0_sod_to_t_end(gpu, oracle_mod, riemann):
+    """BASELINE config 0 in full: N=256 fp64 outflow, CFL 0.4, run to t = 0.2 with the last step clamped (R18)."""
+    w = inputs.baseline_config(0)
+    o = oracle_mod.Oracle(w.n, w.extent, w.gamma, w.dtype, w.boundary, riemann)
+    o.set_state(w.U)
+    k, t = o.run(w.cfl, 100000, w.t_end)
+    ref = o.get_state()
+    for variant in VARIANTS:
+        with gpu.ParaisoHydro(w.n, w.extent, w.gamma, w.dtype, w.boundary, riemann, variant) as h:
+            h.set_state(w.U)
+            kg, tg = h.run(w.cfl, 100000, w.t_end)
+            got = h.get_state()
+        assert (kg, tg) == (k, t) and t == 0.2, (variant, kg, k, tg, t)
+        assert 250 <= k <= 320
+        assert np.all(field_errors(got, ref) <= 1e-9), variant
+
+
+def test_sod_embedded_along_each_axis_is_identical_on_the_gpu(gpu):
+    """P8 on the GPU: a 1-D problem along x, y or z of a 3-D grid reproduces the 1-D run bit for bit."""
+    w1 = inputs.sod(64)
+    with gpu.ParaisoHydro(w1.n, w1.extent, w1.gamma, w1.dtype, "outflow") as h:
+        h.set_state(w1.U)
+        h.run(0.4, 20)
+        ref = h.get_state()
+    for axis in range(3):
+        w3 = inputs.sod(64, axis=axis, dims=3, n_other=5)
+        for variant in VARIANTS:
+            with gpu.ParaisoHydro(w3.n, w3.extent, w3.gamma, w3.dtype, "outflow", "hllc", variant) as h:
+                h.set_state(w3.U)
+                h.run(0.4, 20)
+                got = h.get_state()
+            line = np.moveaxis(got, 3 - axis, -1)  # axes are [f][z][y][x]
+            assert np.array_equal(line[0, 0, 0], ref[0])
+            assert np.array_equal(line[1 + axis, 0, 0], ref[1])
+            assert np.array_equal(line[4, 0, 0], ref[2])
+            assert np.ptp(line[0], axis=(0, 1)).max() == 0
+
+
+def test_abi_error_paths_and_pointer_kinds(gpu):
+    import torch
+
+    w = inputs.random_smooth((32, 24), np.float32, seed=1)
+    h = gpu.ParaisoHydro(w.n, w.extent, w.gamma, w.dtype)
+    with pytest.raises(gpu.ParaisoError) as ei:
+        h.step(1e-3)
+    assert ei.value.code == gpu.PARAISO_ESTATE
+    with pytest.raises(gpu.ParaisoError):
+        h.cfl_dt(0.4)
+    with pytest.raises(gpu.ParaisoError):
+        h.set_option("no_such_option", 1)
+    with pytest.raises(gpu.ParaisoError):
+        h.set_option("variant", 17)
+    h.set_state(w.U)  # host pointer
+    with pytest.raises(gpu.ParaisoError):
+        h.step(float("nan"))
+    with pytest.raises(gpu.ParaisoError):
+        h.step(-1.0)
+    dt = h.cfl_dt(0.4)
+    s = torch.cuda.Stream()
+    h.set_stream(s)
+    h.step(dt)
+    out_dev = torch.empty(w.U.shape, dtype=torch.float32, device="cuda")
+    h.get_state(out_dev)  # device pointer, asynchronous on the handle's stream
+    h.sync()
+    out_host = h.get_state()
+    assert np.array_equal(out_dev.cpu().numpy(), out_host)
+    assert h.launch_count() >= 4
+    assert h.version().startswith("paraiso_hydro")
+    h.destroy()
+    h.destroy()  # idempotent
+
+
+def test_nonfinite_counter_reports_a_broken_state(gpu):
+    w = inputs.random_smooth((40, 40), np.float64, seed=2)
+    U = w.U.copy()
+    U[3, 7, 9] = -5.0  # negative energy -> negative pressure
+    with gpu.ParaisoHydro(w.n, w.extent, w.gamma, w.dtype) as h:
+        h.set_state(U)
+        assert h.stats() >= 1
