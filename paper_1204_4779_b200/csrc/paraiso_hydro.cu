@@ -14,6 +14,24 @@
 
 using namespace ph;
 
+// the 2-D / 3-D instantiations live in fused_<dtype>_d<D>.cu
+namespace ph {
+#define PH_EXTERN1(REAL, DD, RS, ST)                                                                      \
+  extern template bool launch_fused_stage<REAL, DD, RS, ST>(const REAL*, const REAL*, REAL*, const Geom<REAL>&, \
+                                                            Scalars*, cudaStream_t, const int*, int);
+#define PH_EXTERN(REAL, DD)              \
+  PH_EXTERN1(REAL, DD, RIEMANN_HLLC, 1)  \
+  PH_EXTERN1(REAL, DD, RIEMANN_HLLC, 2)  \
+  PH_EXTERN1(REAL, DD, RIEMANN_HLL, 1)   \
+  PH_EXTERN1(REAL, DD, RIEMANN_HLL, 2)
+PH_EXTERN(float, 2)
+PH_EXTERN(float, 3)
+PH_EXTERN(double, 2)
+PH_EXTERN(double, 3)
+#undef PH_EXTERN
+#undef PH_EXTERN1
+}  // namespace ph
+
 enum { VARIANT_FUSED = 0, VARIANT_MANIFEST_FLUX = 1, VARIANT_MANIFEST_ALL = 2, VARIANT_DELAYED = 3 };
 
 struct paraiso_hydro {
@@ -219,7 +237,7 @@ struct Launch {
       }
       case VARIANT_FUSED:
         if (launch_fused_stage<Real, D, RS, STAGE>(Uin, (const Real*)h->U[0], Uout, g, h->sc, h->stream, h->block,
-                                                   h->tile_depth, h->cells_per_thread)) {
+                                                   h->tile_depth)) {
           h->launches += 1;
           break;
         }
