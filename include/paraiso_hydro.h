@@ -121,6 +121,12 @@ int paraiso_hydro_launch_count(paraiso_hydro_t *h, int64_t *launches);
  * Either pointer may be NULL. */
 int paraiso_hydro_kernel_time(paraiso_hydro_t *h, int enable, double *total_ms, int64_t *stage_launches);
 
+/* Test hook: evaluates the hot path's division and square root (DESIGN.md §4 "div_rn / sqrt_rn": the
+ * fast path of the IEEE sequences without range check) element-wise on DEVICE arrays of n elements of
+ * `dtype`: quot[i] = a[i] / b[i], root[i] = sqrt(|a[i]|).  Runs on the legacy default stream and
+ * blocks.  Used by tests/test_gpu_arith.py to check correct rounding against IEEE over the normal range. */
+int paraiso_hydro_debug_arith(int dtype, int64_t n, const void *a, const void *b, void *quot, void *root);
+
 /* Message for the last error on this handle (or the last create failure when h == NULL).  Never NULL. */
 const char *paraiso_hydro_last_error(const paraiso_hydro_t *h);
 

@@ -43,6 +43,7 @@ SIGNATURES = {
     "paraiso_hydro_stats": (_int, [_vp, _pi64]),
     "paraiso_hydro_launch_count": (_int, [_vp, _pi64]),
     "paraiso_hydro_kernel_time": (_int, [_vp, _int, _pdbl, _pi64]),
+    "paraiso_hydro_debug_arith": (_int, [_int, _i64, _vp, _vp, _vp, _vp]),
     "paraiso_hydro_last_error": (ctypes.c_char_p, [_vp]),
     "paraiso_hydro_version": (ctypes.c_char_p, []),
 }
@@ -90,6 +91,24 @@ def _pointer(a):
         dt = {torch.float32: np.dtype(np.float32), torch.float64: np.dtype(np.float64)}[a.dtype]
         return a.data_ptr(), dt, a.numel()
     raise TypeError(f"unsupported state container {type(a)}")
+
+
+def debug_arith(a, b):
+    """paraiso_hydro_debug_arith on two equal-length device tensors: returns (a / b, sqrt(|a|)) as evaluated by
+    the hot path's div_rn / sqrt_rn (device tensors of the same dtype)."""
+    import torch
+
+    lib = load_library()
+    pa, dt, n = _pointer(a)
+    pb, dtb, nb = _pointer(b)
+    if dt != dtb or n != nb or not a.is_cuda or not b.is_cuda:
+        raise ValueError("debug_arith wants two device tensors of equal dtype and length")
+    q, r = torch.empty_like(a), torch.empty_like(a)
+    torch.cuda.synchronize()
+    rc = lib.paraiso_hydro_debug_arith(0 if dt == np.dtype(np.float32) else 1, n, pa, pb, q.data_ptr(), r.data_ptr())
+    if rc != PARAISO_OK:
+        raise ParaisoError(rc, lib.paraiso_hydro_last_error(None).decode())
+    return q, r
 
 
 class ParaisoHydro:

@@ -289,6 +289,15 @@ static void dispatch(paraiso_hydro* h, F&& f) {
 #undef PH_CASE
 }
 
+// the hot path's division and square root (hydro_math.cuh div_rn / sqrt_rn), exposed for tests
+template <class Real>
+__global__ void k_debug_arith(long long n, const Real* a, const Real* b, Real* quot, Real* root) {
+  const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  quot[i] = div_rn(a[i], b[i]);
+  root[i] = sqrt_rn(rabs(a[i]));
+}
+
 static int check_launch(paraiso_hydro* h) {
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail(h, PARAISO_ECUDA, std::string("kernel launch: ") + cudaGetErrorString(e));
@@ -622,6 +631,21 @@ int paraiso_hydro_kernel_time(paraiso_hydro_t* h, int enable, double* total_ms, 
   }
   if (total_ms) *total_ms = h->timed_ms;
   if (stage_launches) *stage_launches = h->timed_count;
+  return PARAISO_OK;
+}
+
+int paraiso_hydro_debug_arith(int dtype, int64_t n, const void* a, const void* b, void* quot, void* root) {
+  if (n < 0 || !a || !b || !quot || !root) return fail(nullptr, PARAISO_EINVAL, "debug_arith: bad argument");
+  if (dtype != PARAISO_F32 && dtype != PARAISO_F64) return fail(nullptr, PARAISO_EINVAL, "debug_arith: bad dtype");
+  if (n == 0) return PARAISO_OK;
+  const unsigned int blocks = (unsigned int)((n + 255) / 256);
+  if (dtype == PARAISO_F32)
+    k_debug_arith<float><<<blocks, 256>>>((long long)n, (const float*)a, (const float*)b, (float*)quot, (float*)root);
+  else
+    k_debug_arith<double><<<blocks, 256>>>((long long)n, (const double*)a, (const double*)b, (double*)quot, (double*)root);
+  cudaError_t e = cudaGetLastError();
+  if (e == cudaSuccess) e = cudaDeviceSynchronize();
+  if (e != cudaSuccess) return fail(nullptr, PARAISO_ECUDA, std::string("debug_arith: ") + cudaGetErrorString(e));
   return PARAISO_OK;
 }
 

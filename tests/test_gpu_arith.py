@@ -1,0 +1,44 @@
+"""The hot path's division and square root (csrc/hydro_math.cuh div_rn / sqrt_rn) against IEEE-754.
+
+DESIGN.md §4: the kernels use the fast path of the IEEE sequences without the range check; inside the
+normal range the result must be the correctly rounded one, i.e. identical to what the oracle's `/` and
+`std::sqrt` produce on the host.  NumPy's float32 / float64 `/` and `sqrt` are IEEE correctly rounded, so
+they are the reference here (no oracle code involved).
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+
+def _operands(dtype, n, seed, lo_exp, hi_exp):
+    rng = np.random.default_rng(seed)
+    mant = rng.uniform(1.0, 2.0, n)
+    e = rng.integers(lo_exp, hi_exp + 1, n)
+    sign = rng.choice([-1.0, 1.0], n)
+    return (sign * np.ldexp(mant, e)).astype(dtype)
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_div_and_sqrt_are_correctly_rounded_in_the_normal_range(dtype):
+    import torch
+
+    from paper_1204_4779_b200 import binding
+
+    n = 1 << 22
+    for seed, (lo, hi) in enumerate([(-2, 2), (-20, 20), (-60, 60)]):
+        a = _operands(dtype, n, 100 + seed, lo, hi)
+        b = _operands(dtype, n, 200 + seed, lo, hi)
+        # a few structured cases: equal operands, near-equal mantissas, zero numerators, powers of two
+        a[:1000] = b[:1000]
+        a[1000:2000] = np.nextafter(b[1000:2000], dtype(np.inf))
+        a[2000:3000] = 0.0
+        b[3000:4000] = np.ldexp(1.0, np.arange(1000) % 41 - 20).astype(dtype)
+        q, r = binding.debug_arith(torch.from_numpy(a).cuda(), torch.from_numpy(b).cuda())
+        q, r = q.cpu().numpy(), r.cpu().numpy()
+        with np.errstate(all="ignore"):
+            qref, rref = a / b, np.sqrt(np.abs(a))
+        nz = a != 0
+        assert np.array_equal(q[nz], qref[nz]), (dtype, lo, hi, int(np.sum(q[nz] != qref[nz])))
+        assert np.all(q[~nz] == 0)
+        assert np.array_equal(r[nz], rref[nz]), (dtype, lo, hi, int(np.sum(r[nz] != rref[nz])))
