@@ -240,25 +240,59 @@ def e2e_run(binding, torch, w, steps, warmup, variant, riemann):
             "d2h_bytes_per_step": nbytes, "ms_per_step": ms / steps, "steps": steps}
 
 
+# Counted arithmetic of DESIGN.md §4 per cell per RK2 step (HLLC; DESIGN.md §8 derives the table): every + - x fma
+# compare select min max abs is one lane-operation, an IEEE division / square root is expanded to the fma sequence the
+# kernels execute (fp32: 1 MUFU + 5 / 4 operations, fp64: 1 MUFU + 7 / 9).  Roofline (b) of north_star = these
+# operations over the FP32 (128 lanes per SM) or FP64 (64 lanes per SM) lane rate of 148 SMs at 1.965 GHz.
+COUNTED_OPS_PER_CELL_STEP = {(1, 4): 299, (2, 4): 638, (3, 4): 1053, (1, 8): 354, (2, 8): 737, (3, 8): 1196}
+SM_COUNT, SM_MAX_GHZ = 148, 1.965
+
+
+def alu_peak_tlaneops(itemsize):
+    return SM_COUNT * (128 if itemsize == 4 else 64) * SM_MAX_GHZ * 1e9 / 1e12
+
+
 def roofline_of(w, r, peak, peak_src, traffic=None):
-    nbytes = 2 * w.nf * w.dtype.itemsize * w.cells  # one stage launch: read the state once, write it once
+    """The slower of north_star's two rooflines is the binding one and is reported as `bound`; the other is kept
+    beside it.  (a) HBM: 2*nf*w*N algorithmic bytes per stage launch (state read once, written once; halo excluded)
+    over the measured copy bandwidth.  (b) ALU: counted lane-operations per stage launch over the FP32 / FP64 lane
+    rate derived from the guide's unit counts and clock."""
+    isz = w.dtype.itemsize
+    nbytes = 2 * w.nf * isz * w.cells
     avg_ms = r["stage_ms"] / max(1, r["stage_launches"])
-    achieved = nbytes / (avg_ms * 1e-3) / 1e9
-    return {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-            "traffic": traffic, "kernel": "RK stage kernel(s) (a1-a5 [+a0 in stage 2])",
-            "algorithmic_bytes_per_launch": nbytes, "avg_launch_ms": avg_ms, "peak_source": peak_src}
+    hbm_achieved = nbytes / (avg_ms * 1e-3) / 1e9
+    ops = COUNTED_OPS_PER_CELL_STEP[(w.dims, isz)] / 2.0 * w.cells
+    alu_achieved = ops / (avg_ms * 1e-3) / 1e12
+    alu_peak = alu_peak_tlaneops(isz)
+    hbm = {"bound": "hbm", "achieved": hbm_achieved, "peak": peak, "unit": "GB/s", "frac": hbm_achieved / peak,
+           "algorithmic_bytes_per_launch": nbytes, "peak_source": peak_src,
+           "gcell_per_s_at_peak": peak * 1e9 / (4 * w.nf * isz) / 1e9}
+    alu = {"bound": "alu", "achieved": alu_achieved, "peak": alu_peak, "unit": "Tlaneop/s", "frac": alu_achieved / alu_peak,
+           "algorithmic_ops_per_launch": ops, "counted_ops_per_cell_step": COUNTED_OPS_PER_CELL_STEP[(w.dims, isz)],
+           "peak_source": "derived: 148 SMs x %d %s lanes x 1.965 GHz (B200_PROFILING.md unit counts and clocks.max.sm)"
+                          % (128 if isz == 4 else 64, "FP32" if isz == 4 else "FP64"),
+           "gcell_per_s_at_peak": alu_peak * 1e12 / COUNTED_OPS_PER_CELL_STEP[(w.dims, isz)] / 1e9}
+    first, other = (alu, hbm) if alu["gcell_per_s_at_peak"] < hbm["gcell_per_s_at_peak"] else (hbm, alu)
+    out = dict(first)
+    out.update({"traffic": traffic, "kernel": "RK stage kernel(s) (a1-a5 [+a0 in stage 2])", "avg_launch_ms": avg_ms,
+                "other_bound": other})
+    return out
 
 
 def ncu_traffic(cfg, variant):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, copied by hand from the
-    committed ncu --set full capture (profiles/traffic.json names the capture); None if not captured."""
-    p = os.path.join(ROOT, "profiles", "traffic.json")
+    committed ncu --set full summary (profiles/traffic.csv names it); None if that variant was not captured."""
+    p = os.path.join(ROOT, "profiles", "traffic.csv")
     if not os.path.exists(p):
         return None
     try:
-        return json.load(open(p)).get(f"config{cfg}:{variant}")
+        for line in open(p).read().splitlines()[1:]:
+            key, val = line.split(",")[:2]
+            if key == f"config{cfg}:{variant}":
+                return float(val)
     except Exception:
-        return None
+        pass
+    return None
 
 
 def main():
@@ -369,7 +403,9 @@ def sweep(binding, torch, args, peak, peak_src):
             rl = roofline_of(w, r, peak, peak_src)
             out.append({"config": cfg, "workload": w.name, "variant": variant, "steps": steps,
                         "value": w.cells * steps / (r["ms"] * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": r["ms"] / steps,
-                        "hbm_frac": rl["frac"], "algorithmic_gbs": rl["achieved"], "launches": r["launches"]})
+                        "bound": rl["bound"], "frac": rl["frac"],
+                        "hbm_frac": (rl if rl["bound"] == "hbm" else rl["other_bound"])["frac"],
+                        "alu_frac": (rl if rl["bound"] == "alu" else rl["other_bound"])["frac"], "launches": r["launches"]})
         del w
     return out
 
