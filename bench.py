@@ -295,6 +295,21 @@ def ncu_traffic(cfg, variant):
     return None
 
 
+def replicas_aggregate(ms_local, cells, steps, world, device=None):
+    """Replicas only: every rank advanced its own copy of the workload.  Returns (max-over-ranks
+    device time in ms, whole-job Gcell/s = all ranks' cell updates / that time).  The only collective is this
+    all-reduce(max) of one timing scalar; it works on any torch.distributed backend (NCCL on GPUs, gloo in tests)."""
+    ms = float(ms_local)
+    if world > 1:
+        import torch
+        import torch.distributed as dist
+
+        t = torch.tensor([ms], dtype=torch.float64, device=device if device is not None else "cpu")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    return ms, cells * steps * world / (ms * 1e-3) / 1e9
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -347,21 +362,12 @@ def main():
     t1 = time.time()
     barrier()
     clocks = sampler.stop(t0, t1) if sampler else None
-    ms = r["ms"]
-    if world > 1:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = w.cells * args.steps * world / (ms * 1e-3) / 1e9
+    ms, value = replicas_aggregate(r["ms"], w.cells, args.steps, world, "cuda")
 
     e2e = None
     if not args.no_e2e:
         e = e2e_run(binding, torch, w, min(args.steps, 5), min(args.warmup, 2), args.variant, args.riemann)
-        ev = e["value"] * world
-        if world > 1:
-            t = torch.tensor([e["ms_per_step"]], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ev = w.cells * world / (float(t.item()) * 1e-3) / 1e9
+        _, ev = replicas_aggregate(e["ms_per_step"], w.cells, 1, world, "cuda")
         e2e = dict(e, value=ev, h2d_bytes_per_step=e["h2d_bytes_per_step"] * world,
                    d2h_bytes_per_step=e["d2h_bytes_per_step"] * world)
 
