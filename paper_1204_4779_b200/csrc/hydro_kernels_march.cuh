@@ -1,0 +1,563 @@
+// hydro_kernels_march.cuh — the fused RK-stage kernel, second design ("march"): ONE kernel per RK stage,
+// every intermediate on chip and computed once per cell / face (Fig. 6-7 :435-472 rebuilt for
+// sm_100a), organised around what the r1b Nsight capture of k_fused showed (profiles/r1b_README.md):
+// the stage is bound by instruction issue, not by DRAM.
+//
+//   * T = f32x2: a thread owns TWO x-adjacent cells, held in 64-bit register pairs and computed with the
+//     packed FADD2 / FMUL2 / FFMA2 instructions (one issue slot, two IEEE-rounded fp32 results, bit-identical
+//     to the scalar instructions); global and shared accesses of the pair are 64-bit; index arithmetic,
+//     loop overhead and register moves are paid once per two cells.  T = float / double: one cell per thread.
+//   * a block = NWX x TY "main" warps (a tile of TXC = NWX*32*W cells by TY rows of the leading plane, marched
+//     through `depth` planes of the last axis with a rolling register window, as in k_fused) + ONE halo warp.
+//     The halo warp loads the 2-cell star halo of every plane, converts it to primitives, and computes the
+//     faces the tile cannot get from its own cells (the flux through the tile's low x / y faces, the low-side
+//     state of the first cell beyond its high x / y faces), so the main warps all do the same work and the two
+//     block barriers per plane no longer wait for stragglers.
+//   * x-neighbours inside a warp exchange face states and fluxes by warp shuffle; only warp-edge lanes and the
+//     y direction go through shared memory.
+//   * Eq. 23 is applied in the order x, y, z onto U_base (R11); the last stage forms the primitives
+//     of the new state in registers and feeds the CFL max (a0) into the block reduction.
+// Ragged tiles and periodic / outflow ghosts need no special cases: a plane position whose global index g lies
+// outside [0, n) holds the state of a mapped cell (wrap or clamp); threads whose own cells lie outside the grid
+// compute but never store.  T = f32x2 needs an even n_x (the launcher falls back to T = float otherwise).
+#pragma once
+#include "hydro_kernels_basic.cuh"
+
+namespace ph {
+
+// ---------------------------------------------------------------- lane helpers
+__device__ __forceinline__ float lane_first(float a) { return a; }
+__device__ __forceinline__ double lane_first(double a) { return a; }
+__device__ __forceinline__ float lane_first(f32x2 a) { return a.v.x; }
+__device__ __forceinline__ float lane_last(float a) { return a; }
+__device__ __forceinline__ double lane_last(double a) { return a; }
+__device__ __forceinline__ float lane_last(f32x2 a) { return a.v.y; }
+// the x-neighbour views of a thread's cells: (left neighbour, own cells but the last) / (own cells but the first, right)
+__device__ __forceinline__ float xshift_left(float, float nb) { return nb; }
+__device__ __forceinline__ double xshift_left(double, double nb) { return nb; }
+__device__ __forceinline__ f32x2 xshift_left(f32x2 own, float nb) { return f32x2(nb, own.v.x); }
+__device__ __forceinline__ float xshift_right(float, float nb) { return nb; }
+__device__ __forceinline__ double xshift_right(double, double nb) { return nb; }
+__device__ __forceinline__ f32x2 xshift_right(f32x2 own, float nb) { return f32x2(own.v.y, nb); }
+// two independent scalars as the lanes of one value (W = 1: the first only)
+__device__ __forceinline__ float lane_pack(float a, float, float*) { return a; }
+__device__ __forceinline__ double lane_pack(double a, double, double*) { return a; }
+__device__ __forceinline__ f32x2 lane_pack(float a, float b, f32x2*) { return f32x2(a, b); }
+
+template <class T> __device__ __forceinline__ T lds(const scalar_t<T>* p) { return *p; }
+template <> __device__ __forceinline__ f32x2 lds<f32x2>(const float* p) { return f32x2(*reinterpret_cast<const float2*>(p)); }
+__device__ __forceinline__ void sts(float* p, float v) { *p = v; }
+__device__ __forceinline__ void sts(double* p, double v) { *p = v; }
+__device__ __forceinline__ void sts(float* p, f32x2 v) { *reinterpret_cast<float2*>(p) = v.v; }
+
+template <class T, int D>
+__device__ __forceinline__ Prim<T, D> prim_from_fields(const T (&u)[D + 2]) {
+  Prim<T, D> P;
+  P.rho = u[0];
+#pragma unroll
+  for (int b = 0; b < D; ++b) P.v[b] = u[1 + b];
+  P.p = u[D + 1];
+  return P;
+}
+template <class T, int D>
+__device__ __forceinline__ void prim_to_fields(const Prim<T, D>& P, T (&u)[D + 2]) {
+  u[0] = P.rho;
+#pragma unroll
+  for (int b = 0; b < D; ++b) u[1 + b] = P.v[b];
+  u[D + 1] = P.p;
+}
+
+// flags lanes whose new state is unusable (R19)
+template <class T, int D>
+__device__ __forceinline__ int bad_lanes(const Prim<T, D>& V, T E) {
+  using S = scalar_t<T>;
+  const T zero = T(S(0));
+  return lane_count(m_or(m_or(m_not(gt(V.rho, zero)), m_not(gt(V.p, zero))), m_not(le(rabs(E), T(S(3.0e38))))));
+}
+
+template <class T, int D, int NWX, int TY>
+struct MarchShape {
+  using S = scalar_t<T>;
+  static constexpr int W = LaneTraits<T>::W;
+  static constexpr int NF = D + 2;
+  static constexpr int TXC = NWX * 32 * W;              // cells per tile row
+  static constexpr int PX = TXC + 4;                    // plane row: tile + 2 halo cells on each side
+  static constexpr int PY = (D == 3) ? TY + 4 : 1;
+  static constexpr int OY = (D == 3) ? 2 : 0;           // plane row of the tile's first row
+  static constexpr int NMAIN = NWX * TY * 32;           // main threads; the halo warp follows them
+  static constexpr int NT = NMAIN + 32;
+  static constexpr int XROWS = (D == 3) ? TY : 1;       // tile rows = x halo tasks per plane
+  static constexpr int XTASK_LANES = (XROWS + W - 1) / W;
+  static constexpr int XHALO_LANES = 4 * XROWS / W;     // lanes of the halo warp that load x halo cells
+  static_assert(D == 2 || D == 3, "the marching kernel covers 2-D and 3-D grids");
+  static_assert(D == 3 || TY == 1, "2-D tiles are rows");
+  static_assert(D == 2 || NWX == 1, "3-D tiles are one warp wide");
+  static_assert(D == 2 || TY >= 4, "four different main warps fill the y halo rows");
+  static_assert(XHALO_LANES <= 32 && XTASK_LANES <= 32, "tile too tall for one halo warp");
+  struct Smem {
+    S V[2][NF][PY][PX];                                 // primitives of plane m (double-buffered), halo 2
+    S LOy[(D == 3) ? NF : 1][TY + 1][(D == 3) ? TXC : 2];  // [r]: low-side y state of tile row r (r = TY: halo warp)
+    S Fy[(D == 3) ? NF : 1][TY][(D == 3) ? TXC : 2];    // [r]: flux through the low y face of tile row r (r = 0: halo warp)
+    S LOx[NF][XROWS][NWX + 1];                          // [e]: low-side x state of the first cell of warp column e (e = NWX: halo warp)
+    S Fx[NF][XROWS][NWX];                               // [e]: flux through the low x face of warp column e (e = 0: halo warp)
+  };
+};
+
+// position g of a plane axis -> the cell whose state it holds (g >= -2)
+__device__ __forceinline__ int march_src(int g, int n, int boundary) {
+  return map_index(g > n + 1 ? n + 1 : g, n, boundary);
+}
+
+// Where the W cells at x positions g .. g+W-1 (g even for W = 2) of a grid row come from: element offsets inside
+// a plane, fixed for the whole march (only the plane changes), so that the index mapping is done once per thread.
+struct CellSrc {
+  int o0, o1;   // first / second cell (o1 unused for W = 1)
+  bool pair;    // W = 2: the two cells are adjacent in memory and 8-byte aligned -> one 64-bit load
+};
+template <class T>
+__device__ __forceinline__ CellSrc cell_src(int g, int rowoff, int nx, int bnd) {
+  CellSrc c;
+  if constexpr (LaneTraits<T>::W == 1) {
+    c.o0 = c.o1 = rowoff + march_src(g, nx, bnd);
+    c.pair = false;
+  } else if (bnd == BOUNDARY_PERIODIC) {
+    int gp = g > nx ? nx : g;  // nx even: (gp, gp+1) wraps as a pair
+    gp = gp < 0 ? gp + nx : (gp >= nx ? gp - nx : gp);
+    c.o0 = rowoff + gp;
+    c.o1 = c.o0 + 1;
+    c.pair = true;
+  } else {
+    c.o0 = rowoff + march_src(g, nx, bnd);
+    c.o1 = rowoff + march_src(g + 1, nx, bnd);
+    c.pair = g >= 0 && g + 1 < nx;
+  }
+  return c;
+}
+// base = element index of the first cell of one field of one plane (all indices fit an int: nf*N < 2^31)
+template <class T>
+__device__ __forceinline__ T ldg_cells(const scalar_t<T>* __restrict__ A, int base, const CellSrc& c) {
+  if constexpr (LaneTraits<T>::W == 1) {
+    return __ldg(A + (base + c.o0));
+  } else {
+    if (c.pair) return f32x2(__ldg(reinterpret_cast<const float2*>(A + (base + c.o0))));
+    return f32x2(__ldg(A + (base + c.o0)), __ldg(A + (base + c.o1)));
+  }
+}
+template <class T>
+__device__ __forceinline__ T ld_cells_rw(const scalar_t<T>* A, int idx) {
+  if constexpr (LaneTraits<T>::W == 1) return A[idx];
+  else return f32x2(*reinterpret_cast<const float2*>(A + idx));
+}
+template <class T>
+__device__ __forceinline__ void st_cells(scalar_t<T>* A, int idx, T v) {
+  if constexpr (LaneTraits<T>::W == 1) A[idx] = v;
+  else *reinterpret_cast<float2*>(A + idx) = v.v;
+}
+__device__ __forceinline__ float shfl_dn(float v) { return __shfl_down_sync(0xffffffffu, v, 1); }
+__device__ __forceinline__ double shfl_dn(double v) { return __shfl_down_sync(0xffffffffu, v, 1); }
+__device__ __forceinline__ float shfl_up(float v) { return __shfl_up_sync(0xffffffffu, v, 1); }
+__device__ __forceinline__ double shfl_up(double v) { return __shfl_up_sync(0xffffffffu, v, 1); }
+
+// All warps of the block arrive at barrier 0 the same number of times, the main warps and the halo warp from
+// different places in the code (PTX bar.sync semantics: arrival is counted per warp, not per call site).
+__device__ __forceinline__ void block_barrier() { asm volatile("bar.sync 0;" ::: "memory"); }
+
+template <class T, int D, int RS, int STAGE, int NWX, int TY, int MINB>
+__global__ void __launch_bounds__(MarchShape<T, D, NWX, TY>::NT, MINB)
+    k_march(const scalar_t<T>* __restrict__ Uin, const scalar_t<T>* Ubase, scalar_t<T>* Uout, Geom<scalar_t<T>> g,
+            Scalars* sc, int depth) {
+  using Sh = MarchShape<T, D, NWX, TY>;
+  using S = scalar_t<T>;
+  using P = Prim<T, D>;
+  constexpr int W = Sh::W, NF = Sh::NF, TXC = Sh::TXC, OY = Sh::OY, XROWS = Sh::XROWS;
+  constexpr int M = D - 1;  // marching axis
+
+  if (sc->done) return;
+  extern __shared__ __align__(16) unsigned char march_smem_raw[];
+  typename Sh::Smem& sm = *reinterpret_cast<typename Sh::Smem*>(march_smem_raw);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int nx = g.n[0], ny = g.n[1], nM = g.n[M], bnd = g.boundary;
+  const int x0 = blockIdx.x * TXC;
+  const int y0 = (D == 3) ? blockIdx.y * TY : 0;
+  const int bm = (D == 3) ? blockIdx.z : blockIdx.y;
+  const int m0 = bm * depth;
+  const int m1 = min(m0 + depth, nM);
+  const int Ni = int(g.N);                              // every element index fits an int: nf*N < 2^31 (create)
+  const int psi = (D == 3) ? nx * ny : nx;              // cells per plane
+  auto plane_of = [&](int m) { return map_index(m, nM, bnd) * psi; };
+  auto grid_row = [&](int gj) { return (D == 3) ? march_src(gj, ny, bnd) * nx : 0; };
+
+  S s_max = S(0);
+  int bad = 0;
+
+  if (warp < NWX * TY) {
+    // =========================================================================== main warps
+    const int row = (D == 3) ? warp : 0;
+    const int wx = (D == 3) ? 0 : warp;
+    const int c0 = (wx * 32 + lane) * W;  // first own cell, tile coordinates
+    const int gi = x0 + c0, gj = y0 + row;
+    const bool active = gi < nx && (D == 2 || gj < ny);
+    const CellSrc src = cell_src<T>(gi, grid_row(gj), nx, bnd);
+    const int own = (D == 3 ? gj * nx : 0) + gi;  // valid when active
+    const int pr = row + OY, pc = c0 + 2;         // own position in the shared plane
+    // 3-D: the first two and the last two main warps also fill one y halo row of the plane each
+    const int yh_py = (D == 3) ? (row == 0 ? 0 : row == 1 ? 1 : row == TY - 2 ? TY + 2 : row == TY - 1 ? TY + 3 : -1) : -1;
+    const bool yh = yh_py >= 0;
+    const CellSrc yh_src = cell_src<T>(gi, grid_row(y0 + (yh ? yh_py : 2) - 2), nx, bnd);
+
+    auto load_cells_of = [&](const CellSrc& c, int m, T (&u)[NF]) {
+      const int pl = plane_of(m);
+#pragma unroll
+      for (int f = 0; f < NF; ++f) u[f] = ldg_cells<T>(Uin, f * Ni + pl, c);
+    };
+    auto sts_plane = [&](int b, int py, const P& V) {
+      T u[NF];
+      prim_to_fields<T, D>(V, u);
+#pragma unroll
+      for (int f = 0; f < NF; ++f) sts(&sm.V[b][f][py][pc], u[f]);
+    };
+
+    const S lam0 = S(sc->lam[STAGE - 1][0]);
+    const S lam1 = S(sc->lam[STAGE - 1][1]);
+    const S lam2 = (D == 3) ? S(sc->lam[STAGE - 1][2]) : S(0);
+
+    // ---- prologue: rolling window at m0
+    P Vc, Vp1, hiM;
+    T Fprev[NF], Unext[NF];
+    {
+      T u[NF];
+      load_cells_of(src, m0 - 2, u);
+      const P Vm2 = prim_of<T, D>(u, g.gm1);
+      load_cells_of(src, m0 - 1, u);
+      const P Vm1 = prim_of<T, D>(u, g.gm1);
+      load_cells_of(src, m0, u);
+      Vc = prim_of<T, D>(u, g.gm1);
+      load_cells_of(src, m0 + 1, u);
+      Vp1 = prim_of<T, D>(u, g.gm1);
+      load_cells_of(src, m0 + 2, Unext);
+      P him1, loc;
+      interpolate<T, D>(Vm2, Vm1, Vc, nullptr, &him1);
+      interpolate<T, D>(Vm1, Vc, Vp1, &loc, &hiM);
+      riemann_flux<T, D, M, RS>(g.gamma, g.igm1, him1, loc, Fprev);
+      sts_plane(0, pr, Vc);
+      if (yh) {
+        load_cells_of(yh_src, m0, u);
+        sts_plane(0, yh_py, prim_of<T, D>(u, g.gm1));
+      }
+    }
+    block_barrier();
+
+    int b = 0;
+    for (int m = m0; m < m1; ++m, b ^= 1) {
+      const bool more = m + 1 < m1;
+      // ------------------------------------------------------------ phase A: slopes, the marching-axis face
+      P hix, lox, hiy;
+      {
+        T vc[NF], l[NF], r[NF];
+        prim_to_fields<T, D>(Vc, vc);
+#pragma unroll
+        for (int f = 0; f < NF; ++f) {
+          l[f] = xshift_left(vc[f], sm.V[b][f][pr][pc - 1]);
+          r[f] = xshift_right(vc[f], sm.V[b][f][pr][pc + W]);
+        }
+        interpolate<T, D>(prim_from_fields<T, D>(l), Vc, prim_from_fields<T, D>(r), &lox, &hix);
+        if (lane == 0) {  // low-side state of this warp column's first cell, for the warp (or halo task) on its left
+          T a[NF];
+          prim_to_fields<T, D>(lox, a);
+#pragma unroll
+          for (int f = 0; f < NF; ++f) sm.LOx[f][row][wx] = lane_first(a[f]);
+        }
+      }
+      if constexpr (D == 3) {
+        T d[NF], u[NF];
+#pragma unroll
+        for (int f = 0; f < NF; ++f) {
+          d[f] = lds<T>(&sm.V[b][f][pr - 1][pc]);
+          u[f] = lds<T>(&sm.V[b][f][pr + 1][pc]);
+        }
+        P loy;
+        interpolate<T, D>(prim_from_fields<T, D>(d), Vc, prim_from_fields<T, D>(u), &loy, &hiy);
+        T a[NF];
+        prim_to_fields<T, D>(loy, a);
+#pragma unroll
+        for (int f = 0; f < NF; ++f) sts(&sm.LOy[f][row][c0], a[f]);
+      }
+      // marching axis: V[m+2], slope of cell m+1, flux through face m+1/2
+      const P Vp2 = prim_of<T, D>(Unext, g.gm1);
+      if (more) load_cells_of(src, m + 3, Unext);
+      P loM1, hiM1;
+      interpolate<T, D>(Vc, Vp1, Vp2, &loM1, &hiM1);
+      T Fnext[NF];
+      riemann_flux<T, D, M, RS>(g.gamma, g.igm1, hiM, loM1, Fnext);
+      if (more) sts_plane(b ^ 1, pr, Vp1);
+      block_barrier();
+
+      // ------------------------------------------------------------ phase B: one Riemann solve per in-plane face
+      T Uy[NF];
+      if (yh && more) load_cells_of(yh_src, m + 1, Uy);
+      T Fx[NF], Fy[NF];
+      {
+        T a[NF], rs[NF];
+        prim_to_fields<T, D>(lox, a);
+#pragma unroll
+        for (int f = 0; f < NF; ++f) {
+          S nb = shfl_dn(lane_first(a[f]));
+          if (lane == 31) nb = sm.LOx[f][row][wx + 1];
+          rs[f] = xshift_right(a[f], nb);
+        }
+        riemann_flux<T, D, 0, RS>(g.gamma, g.igm1, hix, prim_from_fields<T, D>(rs), Fx);
+        if (NWX > 1 && lane == 31 && wx + 1 < NWX) {
+#pragma unroll
+          for (int f = 0; f < NF; ++f) sm.Fx[f][row][wx + 1] = lane_last(Fx[f]);
+        }
+      }
+      if constexpr (D == 3) {
+        T a[NF];
+#pragma unroll
+        for (int f = 0; f < NF; ++f) a[f] = lds<T>(&sm.LOy[f][row + 1][c0]);
+        riemann_flux<T, D, 1, RS>(g.gamma, g.igm1, hiy, prim_from_fields<T, D>(a), Fy);
+        if (row + 1 < TY) {
+#pragma unroll
+          for (int f = 0; f < NF; ++f) sts(&sm.Fy[f][row + 1][c0], Fy[f]);
+        }
+      }
+      // own-cell base state of Eq. 23 (coherent load: the last stage overwrites U_base in place)
+      const int cell = plane_of(m) + own;
+      T u[NF];
+      if (active) {
+#pragma unroll
+        for (int f = 0; f < NF; ++f) u[f] = ld_cells_rw<T>(Ubase, f * Ni + cell);
+      }
+      if (yh && more) sts_plane(b ^ 1, yh_py, prim_of<T, D>(Uy, g.gm1));
+      block_barrier();
+
+      // ------------------------------------------------------------ phase C: Eq. 23, axes in the order x, y, z
+      {
+        T lowx[NF];
+#pragma unroll
+        for (int f = 0; f < NF; ++f) {
+          S nb = shfl_up(lane_last(Fx[f]));
+          if (lane == 0) nb = sm.Fx[f][row][wx];
+          lowx[f] = xshift_left(Fx[f], nb);
+        }
+        if (active) {
+#pragma unroll
+          for (int f = 0; f < NF; ++f) u[f] = rfma(lam0, lowx[f] - Fx[f], u[f]);
+          if constexpr (D == 3) {
+#pragma unroll
+            for (int f = 0; f < NF; ++f) u[f] = rfma(lam1, lds<T>(&sm.Fy[f][row][c0]) - Fy[f], u[f]);
+#pragma unroll
+            for (int f = 0; f < NF; ++f) u[f] = rfma(lam2, Fprev[f] - Fnext[f], u[f]);
+          } else {
+#pragma unroll
+            for (int f = 0; f < NF; ++f) u[f] = rfma(lam1, Fprev[f] - Fnext[f], u[f]);
+          }
+#pragma unroll
+          for (int f = 0; f < NF; ++f) st_cells<T>(Uout, f * Ni + cell, u[f]);
+          if (STAGE == 2) {
+            T ir;
+            const P Vn = prim_of<T, D>(u, g.gm1, &ir);
+            s_max = rmax(s_max, lane_max(cfl_speed<T, D>(Vn, ir, g.gamma, g.idr)));
+            bad += bad_lanes<T, D>(Vn, u[NF - 1]);
+          }
+        }
+      }
+#pragma unroll
+      for (int f = 0; f < NF; ++f) Fprev[f] = Fnext[f];
+      Vc = Vp1;
+      Vp1 = Vp2;
+      hiM = hiM1;
+    }
+  } else {
+    // =========================================================================== the halo warp
+    // It loads the x halo cells of every plane (the y halo rows are filled by four of the main warps) and
+    // computes the faces the tile cannot get from its own cells.  Its face tasks read only the shared plane and
+    // the low-side states the main warps publish, so it never waits for anything but the block barriers.
+    int r, px;
+    if (W == 2) {
+      r = lane >> 1;
+      px = (lane & 1) ? TXC + 2 : 0;
+    } else {
+      r = lane >> 2;
+      px = (lane & 3) < 2 ? (lane & 3) : TXC + (lane & 3);
+    }
+    const bool hval = lane < Sh::XHALO_LANES;
+    r = hval ? r : 0;
+    const int hpy = r + OY, hpx = px;
+    const CellSrc hsrc = cell_src<T>(x0 + px - 2, grid_row(y0 + r), nx, bnd);
+    T Uh[NF];
+    auto load_halo = [&](int m) {
+      const int pl = plane_of(m);
+#pragma unroll
+      for (int f = 0; f < NF; ++f) Uh[f] = ldg_cells<T>(Uin, f * Ni + pl, hsrc);
+    };
+    auto store_halo = [&](int b) {
+      T u[NF];
+      prim_to_fields<T, D>(prim_of<T, D>(Uh, g.gm1), u);
+#pragma unroll
+      for (int f = 0; f < NF; ++f) sts(&sm.V[b][f][hpy][hpx], u[f]);
+    };
+    // x face tasks: lane l < XTASK_LANES handles tile rows ra (first lane of T) and rb (second lane)
+    const bool xtask = lane < Sh::XTASK_LANES;
+    const int ra = xtask ? lane : 0;
+    const int rb = (W == 2) ? min(ra + Sh::XTASK_LANES, XROWS - 1) : ra;
+    auto plane_x = [&](int b, int qx) {
+      T u[NF];
+#pragma unroll
+      for (int f = 0; f < NF; ++f) u[f] = lane_pack(sm.V[b][f][ra + OY][qx], sm.V[b][f][rb + OY][qx], (T*)nullptr);
+      return prim_from_fields<T, D>(u);
+    };
+    auto plane_y = [&](int b, int py) {
+      T u[NF];
+#pragma unroll
+      for (int f = 0; f < NF; ++f) u[f] = lds<T>(&sm.V[b][f][py][lane * W + 2]);
+      return prim_from_fields<T, D>(u);
+    };
+
+    if (hval) {
+      load_halo(m0);
+      store_halo(0);
+    }
+    block_barrier();
+
+    int b = 0;
+    for (int m = m0; m < m1; ++m, b ^= 1) {
+      const bool more = m + 1 < m1;
+      // ---- phase A: high-side states of the cells just below the tile, low-side states of those just above
+      if (hval && more) load_halo(m + 1);
+      P hiYlow, hiXlow;
+      if constexpr (D == 3) {
+        interpolate<T, D>(plane_y(b, 0), plane_y(b, 1), plane_y(b, 2), nullptr, &hiYlow);
+        P lo;
+        interpolate<T, D>(plane_y(b, TY + 1), plane_y(b, TY + 2), plane_y(b, TY + 3), &lo, nullptr);
+        T a[NF];
+        prim_to_fields<T, D>(lo, a);
+#pragma unroll
+        for (int f = 0; f < NF; ++f) sts(&sm.LOy[f][TY][lane * W], a[f]);
+      }
+      if (xtask) {
+        interpolate<T, D>(plane_x(b, 0), plane_x(b, 1), plane_x(b, 2), nullptr, &hiXlow);
+        P lo;
+        interpolate<T, D>(plane_x(b, TXC + 1), plane_x(b, TXC + 2), plane_x(b, TXC + 3), &lo, nullptr);
+        T a[NF];
+        prim_to_fields<T, D>(lo, a);
+#pragma unroll
+        for (int f = 0; f < NF; ++f) {
+          sm.LOx[f][ra][NWX] = lane_first(a[f]);
+          if (W == 2) sm.LOx[f][rb][NWX] = lane_last(a[f]);
+        }
+      }
+      block_barrier();
+      // ---- phase B: flux through the tile's low faces (low-side state from the tile's first row / column);
+      //      primitives of the next plane's x halo
+      if constexpr (D == 3) {
+        T a[NF], F[NF];
+#pragma unroll
+        for (int f = 0; f < NF; ++f) a[f] = lds<T>(&sm.LOy[f][0][lane * W]);
+        riemann_flux<T, D, 1, RS>(g.gamma, g.igm1, hiYlow, prim_from_fields<T, D>(a), F);
+#pragma unroll
+        for (int f = 0; f < NF; ++f) sts(&sm.Fy[f][0][lane * W], F[f]);
+      }
+      if (xtask) {
+        T a[NF], F[NF];
+#pragma unroll
+        for (int f = 0; f < NF; ++f) a[f] = lane_pack(sm.LOx[f][ra][0], sm.LOx[f][rb][0], (T*)nullptr);
+        riemann_flux<T, D, 0, RS>(g.gamma, g.igm1, hiXlow, prim_from_fields<T, D>(a), F);
+#pragma unroll
+        for (int f = 0; f < NF; ++f) {
+          sm.Fx[f][ra][0] = lane_first(F[f]);
+          if (W == 2) sm.Fx[f][rb][0] = lane_last(F[f]);
+        }
+      }
+      if (hval && more) store_halo(b ^ 1);
+      block_barrier();
+    }
+  }
+  if (STAGE == 2) {
+    const unsigned int nblocks = gridDim.x * gridDim.y * gridDim.z;
+    block_reduce_and_finalize<S>(s_max, bad, sc, g, nblocks, 1);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+template <class T, int D, int RS, int STAGE, int NWX, int TY, int MINB>
+static bool launch_march_shape(const scalar_t<T>* Uin, const scalar_t<T>* Ubase, scalar_t<T>* Uout,
+                               const Geom<scalar_t<T>>& g, Scalars* sc, cudaStream_t stream, int depth) {
+  using Sh = MarchShape<T, D, NWX, TY>;
+  auto kern = k_march<T, D, RS, STAGE, NWX, TY, MINB>;
+  static bool configured = false;
+  if (!configured) {
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(typename Sh::Smem)) != cudaSuccess)
+      return false;
+    configured = true;
+  }
+  constexpr int M = D - 1;
+  dim3 grid, block(Sh::NT, 1, 1);
+  grid.x = (g.n[0] + Sh::TXC - 1) / Sh::TXC;
+  if (D == 3) {
+    grid.y = (g.n[1] + TY - 1) / TY;
+    grid.z = (g.n[M] + depth - 1) / depth;
+    if (grid.y > 65535u || grid.z > 65535u) return false;
+  } else {
+    grid.y = (g.n[M] + depth - 1) / depth;
+    grid.z = 1;
+    if (grid.y > 65535u) return false;
+  }
+  kern<<<grid, block, sizeof(typename Sh::Smem), stream>>>(Uin, Ubase, Uout, g, sc, depth);
+  return true;
+}
+
+// Planes marched per block when the caller gives none: deep enough that the 4 extra planes of the prologue
+// stay below ~10 % of the work, shallow enough to give every SM several blocks.
+inline int march_default_depth(long long tiles_in_plane, int nM) {
+  int depth = 64;
+  while (depth > 8 && tiles_in_plane * ((nM + depth - 1) / depth) < 4 * 148) depth >>= 1;
+  return depth;
+}
+
+// Returns false when the marching kernel does not cover this shape (the caller falls back).
+//   pack: cells per thread along x (0 = default: 2 for fp32 on an even n_x, else 1)
+//   block[0] (2-D): main warps per block (0 = default); block[1] (3-D): tile rows TY (0 = default)
+template <class Real, int D, int RS, int STAGE>
+bool launch_march_stage(const Real* Uin, const Real* Ubase, Real* Uout, const Geom<Real>& g, Scalars* sc,
+                        cudaStream_t stream, const int* block, int tile_depth, int pack) {
+  if constexpr (D == 1) {
+    return false;
+  } else {
+    constexpr bool can_pack = sizeof(Real) == 4;
+    constexpr int minb = sizeof(Real) == 4 ? 2 : 1;  // one cell per thread in fp32: two blocks per SM (<= 128 registers)
+    const bool packed = can_pack && pack != 1 && (g.n[0] % 2 == 0);
+    if (pack == 2 && !packed) return false;
+    const int w = packed ? 2 : 1;
+    if constexpr (D == 2) {
+      int nwx = block[0] > 0 ? block[0] : 4;
+      const long long tiles = (g.n[0] + nwx * 32 * w - 1) / (nwx * 32 * w);
+      const int depth = tile_depth > 0 ? tile_depth : march_default_depth(tiles, g.n[1]);
+#define PH_SHAPE(NWXV)                                                                                              \
+  if (nwx == NWXV) {                                                                                                \
+    if constexpr (can_pack)                                                                                         \
+      if (packed) return launch_march_shape<f32x2, D, RS, STAGE, NWXV, 1, 1>(Uin, Ubase, Uout, g, sc, stream, depth); \
+    return launch_march_shape<Real, D, RS, STAGE, NWXV, 1, minb>(Uin, Ubase, Uout, g, sc, stream, depth);           \
+  }
+      PH_SHAPE(2) PH_SHAPE(4) PH_SHAPE(8)
+#undef PH_SHAPE
+      return false;
+    } else {
+      const int ty = block[1] > 0 ? block[1] : 7;  // 7 main warps + the halo warp = 256 threads
+      const long long tiles = (long long)((g.n[0] + 32 * w - 1) / (32 * w)) * ((g.n[1] + ty - 1) / ty);
+      const int depth = tile_depth > 0 ? tile_depth : march_default_depth(tiles, g.n[2]);
+#define PH_SHAPE(TYV)                                                                                               \
+  if (ty == TYV) {                                                                                                  \
+    if constexpr (can_pack)                                                                                         \
+      if (packed) return launch_march_shape<f32x2, D, RS, STAGE, 1, TYV, 1>(Uin, Ubase, Uout, g, sc, stream, depth);  \
+    return launch_march_shape<Real, D, RS, STAGE, 1, TYV, minb>(Uin, Ubase, Uout, g, sc, stream, depth);            \
+  }
+      PH_SHAPE(4) PH_SHAPE(7) PH_SHAPE(8)
+#undef PH_SHAPE
+      return false;
+    }
+  }
+}
+
+}  // namespace ph

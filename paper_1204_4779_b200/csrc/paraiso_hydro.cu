@@ -11,6 +11,7 @@
 
 #include "hydro_kernels_basic.cuh"
 #include "hydro_kernels_fused.cuh"
+#include "hydro_kernels_march.cuh"
 
 using namespace ph;
 
@@ -18,7 +19,9 @@ using namespace ph;
 namespace ph {
 #define PH_EXTERN1(REAL, DD, RS, ST)                                                                      \
   extern template bool launch_fused_stage<REAL, DD, RS, ST>(const REAL*, const REAL*, REAL*, const Geom<REAL>&, \
-                                                            Scalars*, cudaStream_t, const int*, int);
+                                                            Scalars*, cudaStream_t, const int*, int);            \
+  extern template bool launch_march_stage<REAL, DD, RS, ST>(const REAL*, const REAL*, REAL*, const Geom<REAL>&, \
+                                                            Scalars*, cudaStream_t, const int*, int, int);
 #define PH_EXTERN(REAL, DD)              \
   PH_EXTERN1(REAL, DD, RIEMANN_HLLC, 1)  \
   PH_EXTERN1(REAL, DD, RIEMANN_HLLC, 2)  \
@@ -32,7 +35,7 @@ PH_EXTERN(double, 3)
 #undef PH_EXTERN1
 }  // namespace ph
 
-enum { VARIANT_FUSED = 0, VARIANT_MANIFEST_FLUX = 1, VARIANT_MANIFEST_ALL = 2, VARIANT_DELAYED = 3 };
+enum { VARIANT_FUSED = 0, VARIANT_MANIFEST_FLUX = 1, VARIANT_MANIFEST_ALL = 2, VARIANT_DELAYED = 3, VARIANT_MARCH = 4 };
 
 struct paraiso_hydro {
   int dims = 0, dtype = 0, nf = 0;
@@ -235,6 +238,13 @@ struct Launch {
         update<STAGE>(h, g, Uout);
         break;
       }
+      case VARIANT_MARCH:
+        if (launch_march_stage<Real, D, RS, STAGE>(Uin, (const Real*)h->U[0], Uout, g, h->sc, h->stream, h->block,
+                                                   h->tile_depth, h->cells_per_thread)) {
+          h->launches += 1;
+          break;
+        }
+        // shapes the packed / marching kernel does not cover: the first fused design
       case VARIANT_FUSED:
         if (launch_fused_stage<Real, D, RS, STAGE>(Uin, (const Real*)h->U[0], Uout, g, h->sc, h->stream, h->block,
                                                    h->tile_depth)) {
@@ -392,7 +402,7 @@ static bool find_option(paraiso_hydro* h, const char* key, OptionRef* ref) {
   };
   const Opt opts[] = {{"boundary", {&h->boundary, 0, 1}},
                       {"riemann", {&h->riemann, 0, 1}},
-                      {"variant", {&h->variant, 0, 3}},
+                      {"variant", {&h->variant, 0, 4}},
                       {"block_x", {&h->block[0], 0, 1024}},
                       {"block_y", {&h->block[1], 0, 1024}},
                       {"block_z", {&h->block[2], 0, 64}},

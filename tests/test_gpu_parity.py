@@ -13,7 +13,7 @@ from paper_1204_4779_b200 import inputs
 
 pytestmark = pytest.mark.gpu
 
-VARIANTS = ["fused", "manifest_flux", "manifest_all", "delayed"]
+VARIANTS = ["march", "fused", "manifest_flux", "manifest_all", "delayed"]
 
 
 @pytest.fixture(scope="module")
@@ -206,3 +206,37 @@ def test_nonfinite_counter_reports_a_broken_state(gpu):
     with gpu.ParaisoHydro(w.n, w.extent, w.gamma, w.dtype) as h:
         h.set_state(U)
         assert h.stats() >= 1
+
+
+# every launch shape of the marching kernel: packed (two cells per thread) and scalar, all tile heights / widths
+MARCH_SHAPES = [(2, {"cells_per_thread": 1, "block_x": 2}), (2, {"cells_per_thread": 2, "block_x": 2}),
+                (2, {"cells_per_thread": 2, "block_x": 8, "tile_depth": 5}), (2, {"cells_per_thread": 1, "block_x": 8}),
+                (3, {"cells_per_thread": 1, "block_y": 4}), (3, {"cells_per_thread": 2, "block_y": 4}),
+                (3, {"cells_per_thread": 2, "block_y": 7, "tile_depth": 3}), (3, {"cells_per_thread": 2, "block_y": 8}),
+                (3, {"cells_per_thread": 1, "block_y": 8, "tile_depth": 4})]
+
+
+@pytest.mark.parametrize("boundary", ["periodic", "outflow"])
+@pytest.mark.parametrize("dims,opts", MARCH_SHAPES)
+def test_march_launch_shapes_match_oracle(gpu, oracle_mod, dims, opts, boundary):
+    # even n_x (the packed kernel needs it), ragged against every tile edge, several tiles per axis
+    shape = {2: (300, 41), 3: (150, 19, 13)}[dims]
+    for dtype in (np.float32, np.float64):
+        if dtype == np.float64 and opts["cells_per_thread"] == 2:
+            continue
+        w = inputs.random_smooth(shape, dtype, seed=11 + dims, boundary=boundary)
+        ref, rdt = oracle_steps(oracle_mod, w, 3)
+        got, gdt = gpu_steps(gpu, w, 3, "march", **opts)
+        tol1, _, toldt = TOL[np.dtype(dtype)]
+        assert np.all(field_errors(got, ref) <= 3 * tol1), (opts, field_errors(got, ref))
+        assert all(abs(a - b) <= toldt * b for a, b in zip(gdt, rdt))
+        assert np.array_equal(got, ref), "the marching kernel states the same arithmetic as the oracle: bit-equal"
+
+
+def test_march_packed_needs_even_nx_and_falls_back(gpu, oracle_mod):
+    w = inputs.random_smooth((151, 37), np.float32, seed=5)
+    ref, _ = oracle_steps(oracle_mod, w, 2)
+    got, _ = gpu_steps(gpu, w, 2, "march")  # default packing: odd n_x -> one cell per thread
+    assert np.array_equal(got, ref)
+    got, _ = gpu_steps(gpu, w, 2, "march", cells_per_thread=2)  # explicit request: falls back to the first fused design
+    assert np.array_equal(got, ref)
