@@ -23,6 +23,10 @@
 #pragma once
 #include "hydro_kernels_basic.cuh"
 
+#ifndef PH_MARCH_MINB
+#define PH_MARCH_MINB 2
+#endif
+
 namespace ph {
 
 // ---------------------------------------------------------------- lane helpers
@@ -92,8 +96,11 @@ struct MarchShape {
   static_assert(D == 2 || D == 3, "the marching kernel covers 2-D and 3-D grids");
   static_assert(D == 3 || TY == 1, "2-D tiles are rows");
   static_assert(D == 2 || NWX == 1, "3-D tiles are one warp wide");
-  static_assert(D == 2 || TY >= 4, "four different main warps fill the y halo rows");
-  static_assert(XHALO_LANES <= 32 && XTASK_LANES <= 32, "tile too tall for one halo warp");
+  // who fills the four y halo rows of the plane: four of the main warps, or the halo warp (which then carries
+  // about as many instructions per plane as a main warp: the four schedulers of the SM stay evenly loaded)
+  static constexpr bool YH_MAIN = false;
+  static_assert(D == 2 || !YH_MAIN || TY >= 4, "four different main warps fill the y halo rows");
+  static_assert(XTASK_LANES <= 32, "tile too tall for one halo warp");
   struct Smem {
     S V[2][NF][PY][PX];                                 // primitives of plane m (double-buffered), halo 2
     S LOy[(D == 3) ? NF : 1][TY + 1][(D == 3) ? TXC : 2];  // [r]: low-side y state of tile row r (r = TY: halo warp)
@@ -160,7 +167,11 @@ __device__ __forceinline__ double shfl_up(double v) { return __shfl_up_sync(0xff
 
 // All warps of the block arrive at barrier 0 the same number of times, the main warps and the halo warp from
 // different places in the code (PTX bar.sync semantics: arrival is counted per warp, not per call site).
+#ifdef PH_EXPERIMENT_NO_BARRIER
+__device__ __forceinline__ void block_barrier() { __syncwarp(); }
+#else
 __device__ __forceinline__ void block_barrier() { asm volatile("bar.sync 0;" ::: "memory"); }
+#endif
 
 template <class T, int D, int RS, int STAGE, int NWX, int TY, int MINB>
 __global__ void __launch_bounds__(MarchShape<T, D, NWX, TY>::NT, MINB)
@@ -202,7 +213,7 @@ __global__ void __launch_bounds__(MarchShape<T, D, NWX, TY>::NT, MINB)
     const int own = (D == 3 ? gj * nx : 0) + gi;  // valid when active
     const int pr = row + OY, pc = c0 + 2;         // own position in the shared plane
     // 3-D: the first two and the last two main warps also fill one y halo row of the plane each
-    const int yh_py = (D == 3) ? (row == 0 ? 0 : row == 1 ? 1 : row == TY - 2 ? TY + 2 : row == TY - 1 ? TY + 3 : -1) : -1;
+    const int yh_py = (D == 3 && Sh::YH_MAIN) ? (row == 0 ? 0 : row == 1 ? 1 : row == TY - 2 ? TY + 2 : row == TY - 1 ? TY + 3 : -1) : -1;
     const bool yh = yh_py >= 0;
     const CellSrc yh_src = cell_src<T>(gi, grid_row(y0 + (yh ? yh_py : 2) - 2), nx, bnd);
 
@@ -374,29 +385,61 @@ __global__ void __launch_bounds__(MarchShape<T, D, NWX, TY>::NT, MINB)
     // It loads the x halo cells of every plane (the y halo rows are filled by four of the main warps) and
     // computes the faces the tile cannot get from its own cells.  Its face tasks read only the shared plane and
     // the low-side states the main warps publish, so it never waits for anything but the block barriers.
-    int r, px;
-    if (W == 2) {
-      r = lane >> 1;
-      px = (lane & 1) ? TXC + 2 : 0;
-    } else {
-      r = lane >> 2;
-      px = (lane & 3) < 2 ? (lane & 3) : TXC + (lane & 3);
+    constexpr int NXP = (Sh::XHALO_LANES + 31) / 32;  // x halo slots per lane
+    CellSrc hsrc[NXP];
+    int hpy[NXP], hpx[NXP];
+    bool hval[NXP];
+#pragma unroll
+    for (int q = 0; q < NXP; ++q) {
+      const int id = lane + 32 * q;
+      int r, px;
+      if (W == 2) {
+        r = id >> 1;
+        px = (id & 1) ? TXC + 2 : 0;
+      } else {
+        r = id >> 2;
+        px = (id & 3) < 2 ? (id & 3) : TXC + (id & 3);
+      }
+      hval[q] = id < Sh::XHALO_LANES;
+      r = hval[q] ? r : 0;
+      hpy[q] = r + OY;
+      hpx[q] = px;
+      hsrc[q] = cell_src<T>(x0 + px - 2, grid_row(y0 + r), nx, bnd);
     }
-    const bool hval = lane < Sh::XHALO_LANES;
-    r = hval ? r : 0;
-    const int hpy = r + OY, hpx = px;
-    const CellSrc hsrc = cell_src<T>(x0 + px - 2, grid_row(y0 + r), nx, bnd);
-    T Uh[NF];
+    constexpr int NYP = (D == 3 && !Sh::YH_MAIN) ? 4 : 0;  // y halo rows this warp fills
+    CellSrc ysrc[NYP > 0 ? NYP : 1];
+#pragma unroll
+    for (int q = 0; q < NYP; ++q) ysrc[q] = cell_src<T>(x0 + lane * W, grid_row(y0 + (q < 2 ? q : TY + q) - 2), nx, bnd);
+    T Uh[NXP][NF], Uyh[NYP > 0 ? NYP : 1][NF];
     auto load_halo = [&](int m) {
       const int pl = plane_of(m);
 #pragma unroll
-      for (int f = 0; f < NF; ++f) Uh[f] = ldg_cells<T>(Uin, f * Ni + pl, hsrc);
+      for (int q = 0; q < NXP; ++q)
+        if (hval[q]) {
+#pragma unroll
+          for (int f = 0; f < NF; ++f) Uh[q][f] = ldg_cells<T>(Uin, f * Ni + pl, hsrc[q]);
+        }
+#pragma unroll
+      for (int q = 0; q < NYP; ++q) {
+#pragma unroll
+        for (int f = 0; f < NF; ++f) Uyh[q][f] = ldg_cells<T>(Uin, f * Ni + pl, ysrc[q]);
+      }
     };
     auto store_halo = [&](int b) {
       T u[NF];
-      prim_to_fields<T, D>(prim_of<T, D>(Uh, g.gm1), u);
 #pragma unroll
-      for (int f = 0; f < NF; ++f) sts(&sm.V[b][f][hpy][hpx], u[f]);
+      for (int q = 0; q < NXP; ++q)
+        if (hval[q]) {
+          prim_to_fields<T, D>(prim_of<T, D>(Uh[q], g.gm1), u);
+#pragma unroll
+          for (int f = 0; f < NF; ++f) sts(&sm.V[b][f][hpy[q]][hpx[q]], u[f]);
+        }
+#pragma unroll
+      for (int q = 0; q < NYP; ++q) {
+        prim_to_fields<T, D>(prim_of<T, D>(Uyh[q], g.gm1), u);
+#pragma unroll
+        for (int f = 0; f < NF; ++f) sts(&sm.V[b][f][q < 2 ? q : TY + q][lane * W + 2], u[f]);
+      }
     };
     // x face tasks: lane l < XTASK_LANES handles tile rows ra (first lane of T) and rb (second lane)
     const bool xtask = lane < Sh::XTASK_LANES;
@@ -415,17 +458,15 @@ __global__ void __launch_bounds__(MarchShape<T, D, NWX, TY>::NT, MINB)
       return prim_from_fields<T, D>(u);
     };
 
-    if (hval) {
-      load_halo(m0);
-      store_halo(0);
-    }
+    load_halo(m0);
+    store_halo(0);
     block_barrier();
 
     int b = 0;
     for (int m = m0; m < m1; ++m, b ^= 1) {
       const bool more = m + 1 < m1;
       // ---- phase A: high-side states of the cells just below the tile, low-side states of those just above
-      if (hval && more) load_halo(m + 1);
+      if (more) load_halo(m + 1);
       P hiYlow, hiXlow;
       if constexpr (D == 3) {
         interpolate<T, D>(plane_y(b, 0), plane_y(b, 1), plane_y(b, 2), nullptr, &hiYlow);
@@ -470,7 +511,7 @@ __global__ void __launch_bounds__(MarchShape<T, D, NWX, TY>::NT, MINB)
           if (W == 2) sm.Fx[f][rb][0] = lane_last(F[f]);
         }
       }
-      if (hval && more) store_halo(b ^ 1);
+      if (more) store_halo(b ^ 1);
       block_barrier();
     }
   }
@@ -526,7 +567,7 @@ bool launch_march_stage(const Real* Uin, const Real* Ubase, Real* Uout, const Ge
     return false;
   } else {
     constexpr bool can_pack = sizeof(Real) == 4;
-    constexpr int minb = sizeof(Real) == 4 ? 2 : 1;  // one cell per thread in fp32: two blocks per SM (<= 128 registers)
+    constexpr int minb = sizeof(Real) == 4 ? PH_MARCH_MINB : 1;  // one cell per thread in fp32: blocks per SM the register cap is set for
     const bool packed = can_pack && pack != 1 && (g.n[0] % 2 == 0);
     if (pack == 2 && !packed) return false;
     const int w = packed ? 2 : 1;
@@ -551,9 +592,9 @@ bool launch_march_stage(const Real* Uin, const Real* Ubase, Real* Uout, const Ge
   if (ty == TYV) {                                                                                                  \
     if constexpr (can_pack)                                                                                         \
       if (packed) return launch_march_shape<f32x2, D, RS, STAGE, 1, TYV, 1>(Uin, Ubase, Uout, g, sc, stream, depth);  \
-    return launch_march_shape<Real, D, RS, STAGE, 1, TYV, minb>(Uin, Ubase, Uout, g, sc, stream, depth);            \
+    return launch_march_shape<Real, D, RS, STAGE, 1, TYV, (TYV > 8 ? 1 : minb)>(Uin, Ubase, Uout, g, sc, stream, depth);            \
   }
-      PH_SHAPE(4) PH_SHAPE(7) PH_SHAPE(8)
+      PH_SHAPE(4) PH_SHAPE(7) PH_SHAPE(8) PH_SHAPE(15)
 #undef PH_SHAPE
       return false;
     }
