@@ -280,6 +280,8 @@ def roofline_of(w, r, peak, peak_src, traffic=None):
 
 
 def ncu_traffic(cfg, variant):
+    if cfg in (1, 2) and variant == "fused":
+        variant = "fused1"  # 2-D grids: the default on-chip variant is k_fused
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, copied by hand from the
     committed ncu --set full summary (profiles/traffic.csv names it); None if that variant was not captured."""
     p = os.path.join(ROOT, "profiles", "traffic.csv")
@@ -400,7 +402,7 @@ def sweep(binding, torch, args, peak, peak_src):
         w = make_workload(cfg)
         big = w.cells >= (1 << 22)
         steps = min(DEFAULT_STEPS[cfg], 100 if not big else 10)
-        for variant in ("fused", "manifest_flux", "manifest_all", "delayed"):
+        for variant in ("fused", "march", "fused1", "manifest_flux", "manifest_all", "delayed"):
             try:
                 r = device_run(binding, torch, w, steps, 3, variant, args.riemann, big)
             except Exception as ex:  # e.g. out of memory for manifest_all

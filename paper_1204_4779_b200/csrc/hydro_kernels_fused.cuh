@@ -348,7 +348,7 @@ bool launch_fused_stage(const Real* Uin, const Real* Ubase, Real* Uout, const Ge
   if constexpr (D == 1) {
     return false;
   } else if constexpr (D == 2) {
-    int tx = block[0] > 0 ? block[0] : (g.n[0] >= 2048 ? 256 : 128);
+    int tx = block[0] > 0 ? block[0] : 128;  // 256-thread rows of the fp64 last stage need 148 registers: one block per SM
     const long long tiles = (g.n[0] + tx - 1) / tx;
     const int depth = tile_depth > 0 ? tile_depth : default_tile_depth(tiles, g.n[1]);
 #define PH_SHAPE(TXV) \

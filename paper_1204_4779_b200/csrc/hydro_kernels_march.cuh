@@ -23,6 +23,12 @@
 #pragma once
 #include "hydro_kernels_basic.cuh"
 
+#ifndef PH_MARCH_UNROLL
+#define PH_MARCH_UNROLL 1
+#endif
+#ifndef PH_MARCH_ZLATE
+#define PH_MARCH_ZLATE 0
+#endif
 #ifndef PH_MARCH_MINB
 #define PH_MARCH_MINB 2
 #endif
@@ -260,6 +266,8 @@ __global__ void __launch_bounds__(MarchShape<T, D, NWX, TY>::NT, MINB)
     block_barrier();
 
     int b = 0;
+    constexpr int unroll_planes = PH_MARCH_UNROLL;
+#pragma unroll unroll_planes
     for (int m = m0; m < m1; ++m, b ^= 1) {
       const bool more = m + 1 < m1;
       // ------------------------------------------------------------ phase A: slopes, the marching-axis face
@@ -299,10 +307,18 @@ __global__ void __launch_bounds__(MarchShape<T, D, NWX, TY>::NT, MINB)
       if (more) load_cells_of(src, m + 3, Unext);
       P loM1, hiM1;
       interpolate<T, D>(Vc, Vp1, Vp2, &loM1, &hiM1);
+#if !PH_MARCH_ZLATE
       T Fnext[NF];
       riemann_flux<T, D, M, RS>(g.gamma, g.igm1, hiM, loM1, Fnext);
+#endif
       if (more) sts_plane(b ^ 1, pr, Vp1);
       block_barrier();
+#if PH_MARCH_ZLATE
+      // the three Riemann solves of a cell are independent dependency chains: issued together they hide each
+      // other's MUFU / FMA latency
+      T Fnext[NF];
+      riemann_flux<T, D, M, RS>(g.gamma, g.igm1, hiM, loM1, Fnext);
+#endif
 
       // ------------------------------------------------------------ phase B: one Riemann solve per in-plane face
       T Uy[NF];
@@ -552,13 +568,14 @@ static bool launch_march_shape(const scalar_t<T>* Uin, const scalar_t<T>* Ubase,
 // Planes marched per block when the caller gives none: deep enough that the 4 extra planes of the prologue
 // stay below ~10 % of the work, shallow enough to give every SM several blocks.
 inline int march_default_depth(long long tiles_in_plane, int nM) {
-  int depth = 64;
+  int depth = 128;
   while (depth > 8 && tiles_in_plane * ((nM + depth - 1) / depth) < 4 * 148) depth >>= 1;
   return depth;
 }
 
 // Returns false when the marching kernel does not cover this shape (the caller falls back).
-//   pack: cells per thread along x (0 = default: 2 for fp32 on an even n_x, else 1)
+//   pack: cells per thread along x (0 = default = 1; 2 = packed f32x2, fp32 on an even n_x only: measured slower,
+//         DESIGN.md §7)
 //   block[0] (2-D): main warps per block (0 = default); block[1] (3-D): tile rows TY (0 = default)
 template <class Real, int D, int RS, int STAGE>
 bool launch_march_stage(const Real* Uin, const Real* Ubase, Real* Uout, const Geom<Real>& g, Scalars* sc,
@@ -568,7 +585,7 @@ bool launch_march_stage(const Real* Uin, const Real* Ubase, Real* Uout, const Ge
   } else {
     constexpr bool can_pack = sizeof(Real) == 4;
     constexpr int minb = sizeof(Real) == 4 ? PH_MARCH_MINB : 1;  // one cell per thread in fp32: blocks per SM the register cap is set for
-    const bool packed = can_pack && pack != 1 && (g.n[0] % 2 == 0);
+    const bool packed = can_pack && pack == 2 && (g.n[0] % 2 == 0);
     if (pack == 2 && !packed) return false;
     const int w = packed ? 2 : 1;
     if constexpr (D == 2) {

@@ -35,7 +35,8 @@ PH_EXTERN(double, 3)
 #undef PH_EXTERN1
 }  // namespace ph
 
-enum { VARIANT_FUSED = 0, VARIANT_MANIFEST_FLUX = 1, VARIANT_MANIFEST_ALL = 2, VARIANT_DELAYED = 3, VARIANT_MARCH = 4 };
+enum { VARIANT_FUSED = 0, VARIANT_MANIFEST_FLUX = 1, VARIANT_MANIFEST_ALL = 2, VARIANT_DELAYED = 3, VARIANT_MARCH = 4,
+       VARIANT_FUSED1 = 5 };
 
 struct paraiso_hydro {
   int dims = 0, dtype = 0, nf = 0;
@@ -238,14 +239,16 @@ struct Launch {
         update<STAGE>(h, g, Uout);
         break;
       }
+      case VARIANT_FUSED:  // the faster of the two on-chip designs per grid kind: 3-D k_march, 2-D k_fused
       case VARIANT_MARCH:
-        if (launch_march_stage<Real, D, RS, STAGE>(Uin, (const Real*)h->U[0], Uout, g, h->sc, h->stream, h->block,
+        if ((h->variant == VARIANT_MARCH || D == 3) &&
+            launch_march_stage<Real, D, RS, STAGE>(Uin, (const Real*)h->U[0], Uout, g, h->sc, h->stream, h->block,
                                                    h->tile_depth, h->cells_per_thread)) {
           h->launches += 1;
           break;
         }
-        // shapes the packed / marching kernel does not cover: the first fused design
-      case VARIANT_FUSED:
+        // shapes the marching kernel does not cover: the first fused design
+      case VARIANT_FUSED1:
         if (launch_fused_stage<Real, D, RS, STAGE>(Uin, (const Real*)h->U[0], Uout, g, h->sc, h->stream, h->block,
                                                    h->tile_depth)) {
           h->launches += 1;
@@ -402,7 +405,7 @@ static bool find_option(paraiso_hydro* h, const char* key, OptionRef* ref) {
   };
   const Opt opts[] = {{"boundary", {&h->boundary, 0, 1}},
                       {"riemann", {&h->riemann, 0, 1}},
-                      {"variant", {&h->variant, 0, 4}},
+                      {"variant", {&h->variant, 0, 5}},
                       {"block_x", {&h->block[0], 0, 1024}},
                       {"block_y", {&h->block[1], 0, 1024}},
                       {"block_z", {&h->block[2], 0, 64}},

@@ -13,7 +13,7 @@ from paper_1204_4779_b200 import inputs
 
 pytestmark = pytest.mark.gpu
 
-VARIANTS = ["march", "fused", "manifest_flux", "manifest_all", "delayed"]
+VARIANTS = ["fused", "march", "fused1", "manifest_flux", "manifest_all", "delayed"]
 
 
 @pytest.fixture(scope="module")
@@ -236,7 +236,7 @@ def test_march_launch_shapes_match_oracle(gpu, oracle_mod, dims, opts, boundary)
 def test_march_packed_needs_even_nx_and_falls_back(gpu, oracle_mod):
     w = inputs.random_smooth((151, 37), np.float32, seed=5)
     ref, _ = oracle_steps(oracle_mod, w, 2)
-    got, _ = gpu_steps(gpu, w, 2, "march")  # default packing: odd n_x -> one cell per thread
+    got, _ = gpu_steps(gpu, w, 2, "march")  # default: one cell per thread
     assert np.array_equal(got, ref)
     got, _ = gpu_steps(gpu, w, 2, "march", cells_per_thread=2)  # explicit request: falls back to the first fused design
     assert np.array_equal(got, ref)
