@@ -384,6 +384,11 @@ def main():
             "roofline": roofline_of(w, r, peak, peak_src, ncu_traffic(args.config, args.variant)),
             "e2e": e2e, "gpu_launches": r["launches"], "clocks": clocks}
 
+    if rank == 0:
+        # measured issue cost (scheduler cycles per instruction) of the instruction classes of the stage kernel on
+        # this device: the model DESIGN.md §8 reads the ncu captures with
+        mhz = (clocks or {}).get("sm_mhz") or 1965.0
+        line["roofline"]["issue_cost_cycles"] = {k: round(binding.debug_issue_cost(k, mhz)[0], 3) for k in binding.ISSUE_KINDS}
     if rank == 0 and not args.no_sweep:
         line["all_configs"] = sweep(binding, torch, args, peak, peak_src)
     if rank == 0 and not args.no_cpu:

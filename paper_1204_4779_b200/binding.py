@@ -44,6 +44,7 @@ SIGNATURES = {
     "paraiso_hydro_launch_count": (_int, [_vp, _pi64]),
     "paraiso_hydro_kernel_time": (_int, [_vp, _int, _pdbl, _pi64]),
     "paraiso_hydro_debug_arith": (_int, [_int, _i64, _vp, _vp, _vp, _vp]),
+    "paraiso_hydro_debug_issue_cost": (_int, [_int, _dbl, _pdbl, _pdbl]),
     "paraiso_hydro_last_error": (ctypes.c_char_p, [_vp]),
     "paraiso_hydro_version": (ctypes.c_char_p, []),
 }
@@ -91,6 +92,21 @@ def _pointer(a):
         dt = {torch.float32: np.dtype(np.float32), torch.float64: np.dtype(np.float64)}[a.dtype]
         return a.data_ptr(), dt, a.numel()
     raise TypeError(f"unsupported state container {type(a)}")
+
+
+ISSUE_KINDS = {"ffma": 0, "fmnmx": 1, "fsetp_fsel": 2, "iadd3_lop3": 3, "ffma2": 4, "dfma": 5, "mufu": 6}
+
+
+def debug_issue_cost(kind, sm_clock_mhz):
+    """paraiso_hydro_debug_issue_cost: (scheduler cycles one more instruction of `kind` costs next to 16 FFMA per
+    iteration, cycles of the 16-FFMA loop alone)."""
+    lib = load_library()
+    c, base = _dbl(0.0), _dbl(0.0)
+    rc = lib.paraiso_hydro_debug_issue_cost(ISSUE_KINDS[kind] if isinstance(kind, str) else int(kind), float(sm_clock_mhz),
+                                            ctypes.byref(c), ctypes.byref(base))
+    if rc:
+        raise ParaisoError(rc, "debug_issue_cost failed")
+    return c.value, base.value
 
 
 def debug_arith(a, b):

@@ -23,12 +23,6 @@
 #pragma once
 #include "hydro_kernels_basic.cuh"
 
-#ifndef PH_MARCH_UNROLL
-#define PH_MARCH_UNROLL 1
-#endif
-#ifndef PH_MARCH_ZLATE
-#define PH_MARCH_ZLATE 0
-#endif
 #ifndef PH_MARCH_MINB
 #define PH_MARCH_MINB 2
 #endif
@@ -173,7 +167,7 @@ __device__ __forceinline__ double shfl_up(double v) { return __shfl_up_sync(0xff
 
 // All warps of the block arrive at barrier 0 the same number of times, the main warps and the halo warp from
 // different places in the code (PTX bar.sync semantics: arrival is counted per warp, not per call site).
-#ifdef PH_EXPERIMENT_NO_BARRIER
+#ifdef PH_EXPERIMENT_NO_BARRIER  // timing ablation of profiles/r1c_README.md (racy, wrong results); never defined by build.py
 __device__ __forceinline__ void block_barrier() { __syncwarp(); }
 #else
 __device__ __forceinline__ void block_barrier() { asm volatile("bar.sync 0;" ::: "memory"); }
@@ -266,8 +260,6 @@ __global__ void __launch_bounds__(MarchShape<T, D, NWX, TY>::NT, MINB)
     block_barrier();
 
     int b = 0;
-    constexpr int unroll_planes = PH_MARCH_UNROLL;
-#pragma unroll unroll_planes
     for (int m = m0; m < m1; ++m, b ^= 1) {
       const bool more = m + 1 < m1;
       // ------------------------------------------------------------ phase A: slopes, the marching-axis face
@@ -307,18 +299,10 @@ __global__ void __launch_bounds__(MarchShape<T, D, NWX, TY>::NT, MINB)
       if (more) load_cells_of(src, m + 3, Unext);
       P loM1, hiM1;
       interpolate<T, D>(Vc, Vp1, Vp2, &loM1, &hiM1);
-#if !PH_MARCH_ZLATE
       T Fnext[NF];
       riemann_flux<T, D, M, RS>(g.gamma, g.igm1, hiM, loM1, Fnext);
-#endif
       if (more) sts_plane(b ^ 1, pr, Vp1);
       block_barrier();
-#if PH_MARCH_ZLATE
-      // the three Riemann solves of a cell are independent dependency chains: issued together they hide each
-      // other's MUFU / FMA latency
-      T Fnext[NF];
-      riemann_flux<T, D, M, RS>(g.gamma, g.igm1, hiM, loM1, Fnext);
-#endif
 
       // ------------------------------------------------------------ phase B: one Riemann solve per in-plane face
       T Uy[NF];

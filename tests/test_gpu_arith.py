@@ -42,3 +42,27 @@ def test_div_and_sqrt_are_correctly_rounded_in_the_normal_range(dtype):
         assert np.array_equal(q[nz], qref[nz]), (dtype, lo, hi, int(np.sum(q[nz] != qref[nz])))
         assert np.all(q[~nz] == 0)
         assert np.array_equal(r[nz], rref[nz]), (dtype, lo, hi, int(np.sum(r[nz] != rref[nz])))
+
+
+def test_issue_cost_of_the_instruction_classes():
+    """DESIGN.md §8 reads the ncu captures with this model: an FFMA costs one scheduler cycle, an ALU-pipe
+    instruction (FMNMX, FSETP, FSEL, IADD3, LOP3) about two even with FFMA work to overlap, a packed FFMA2 two
+    (two results: half the issue slots per result), a DFMA two.  Measured on the device under test."""
+    import subprocess
+
+    from paper_1204_4779_b200 import binding
+
+    try:
+        mhz = float(subprocess.run(["nvidia-smi", "--query-gpu=clocks.max.sm", "--format=csv,noheader,nounits", "-i", "0"],
+                                   capture_output=True, text=True, timeout=30).stdout.split()[0])
+    except Exception:
+        mhz = 1965.0
+    cost = {k: binding.debug_issue_cost(k, mhz)[0] for k in binding.ISSUE_KINDS}
+    base = binding.debug_issue_cost("ffma", mhz)[1]
+    print("issue cost in scheduler cycles per instruction:", {k: round(v, 2) for k, v in cost.items()}, "16-FFMA loop:", round(base, 1))
+    assert 16.0 <= base <= 30.0            # 16 FFMA + loop control at about one instruction per cycle
+    assert 0.8 <= cost["ffma"] <= 1.4
+    for k in ("fmnmx", "fsetp_fsel", "iadd3_lop3"):
+        assert 1.4 <= cost[k] <= 2.6, (k, cost[k])
+    assert 1.6 <= cost["ffma2"] <= 2.6 and 1.6 <= cost["dfma"] <= 2.6
+    assert cost["mufu"] >= 1.6
