@@ -70,7 +70,10 @@ int paraiso_hydro_destroy(paraiso_hydro_t *h);
  *               2 manifest_all   V, VL/VR and F_a all materialised in HBM, one kernel per piece
  *               3 delayed     one kernel per stage, every thread recomputes all it needs from U
  *   "block_x" "block_y" "block_z" "tile_depth" "cells_per_thread"   launch-shape knobs of the sweep (0 = default)
- *   "graph"     1 replay steps of run() from a captured CUDA graph (default) | 0 plain launches */
+ *   "graph"     1 replay steps of run() from a captured CUDA graph (default) | 0 plain launches
+ *   "state_kind" 0 set_state / get_state exchange conserved variables U = (rho, m_a, E) (default) |
+ *               1 primitive variables V = (rho, v_a, p): converted on the device with the EOS of PAPER.md:694
+ *               (set_state) and by Eq. 19 (get_state); the state inside the handle is always conserved */
 int paraiso_hydro_set_option(paraiso_hydro_t *h, const char *key, int64_t value);
 int paraiso_hydro_get_option(paraiso_hydro_t *h, const char *key, int64_t *value);
 

@@ -26,6 +26,8 @@ def _lib(kind="serial"):
         L.oracle_set_option.argtypes = [vp, ctypes.c_char_p, i64]
         L.oracle_set_state.argtypes = [vp, vp]
         L.oracle_get_state.argtypes = [vp, vp]
+        L.oracle_set_primitive.argtypes = [vp, vp]
+        L.oracle_get_primitive.argtypes = [vp, vp]
         L.oracle_cfl_dt.argtypes = [vp, dbl]
         L.oracle_cfl_dt.restype = dbl
         L.oracle_step.argtypes = [vp, dbl]
@@ -68,6 +70,17 @@ class Oracle:
     def get_state(self):
         out = np.empty(self.shape, self.dtype)
         self._L.oracle_get_state(self._h, out.ctypes.data)
+        return out
+
+    def set_primitive(self, V):
+        """V = (rho, v_a, p), same layout as the state: converted with the EOS of PAPER.md:694 (DESIGN.md §4 "cons")."""
+        V = np.ascontiguousarray(V, dtype=self.dtype)
+        assert V.shape == self.shape, (V.shape, self.shape)
+        self._L.oracle_set_primitive(self._h, V.ctypes.data)
+
+    def get_primitive(self):
+        out = np.empty(self.shape, self.dtype)
+        self._L.oracle_get_primitive(self._h, out.ctypes.data)
         return out
 
     def cfl_dt(self, cfl):

@@ -28,7 +28,8 @@
 // tests/golden/sod_n8_first_stage.txt), stationary contact (P4), Sod against the exact Riemann
 // solution (P5), the paper's entropy-wave and sound-wave tests Eq. 28-29 with ~2nd-order
 // convergence (P6, P7), x/y/z embedding identity (P8), mirror symmetry (P9), Riemann-solver
-// special cases (P10), an independent NumPy restatement on <= 8 cells (P11).
+// special cases (P10), an independent NumPy restatement on <= 8 cells (P11), primitive <-> conserved
+// conversion against closed forms and its round trip (P13).
 // Every exported function below is pinned by at least one of these; nothing here is "parity
 // unpinned".  (Unpinned, because absent from the text: the error curves of the paper's Fig. 10.)
 //
@@ -111,6 +112,32 @@ struct Solver {
     V.rho = rho;
     V.p = gm1 * std::fma(-(Real(0.5) * rho), q, E);
     return V;
+  }
+
+  // The inverse of Eq. 19: U = (rho, rho v_a, E) with the EOS E = p/(gamma-1) + rho v^2/2, written
+  // as in DESIGN.md §4 "cons": q as in prim_of, E = fma(0.5 rho, q, p igm1).  Used when a caller hands over
+  // primitive variables (state_kind = 1 of the C ABI); pinned by closed-form values and the round trip (P13).
+  void set_primitive(const Real* V) {
+    for (int64_t c = 0; c < N; ++c) {
+      const Real rho = V[c];
+      Real q = Real(0);
+      for (int b = 0; b < D; ++b) {
+        const Real vb = V[size_t(1 + b) * N + c];
+        q = b == 0 ? vb * vb : std::fma(vb, vb, q);
+        U[size_t(1 + b) * N + c] = rho * vb;
+      }
+      U[c] = rho;
+      U[size_t(D + 1) * N + c] = std::fma(Real(0.5) * rho, q, V[size_t(D + 1) * N + c] * igm1);
+    }
+    t = 0.0;
+  }
+  void get_primitive(Real* V) const {
+    for (int64_t c = 0; c < N; ++c) {
+      const Prim<Real> P = prim_of(U.data(), c);
+      V[c] = P.rho;
+      for (int b = 0; b < D; ++b) V[size_t(1 + b) * N + c] = P.v[b];
+      V[size_t(D + 1) * N + c] = P.p;
+    }
   }
 
   // Eq. 21, literal order of the three cases (R9).
@@ -367,6 +394,24 @@ int oracle_get_state(void* hv, void* U) {
   Handle* h = static_cast<Handle*>(hv);
   return dispatch(h, [&](auto* s) {
     std::memcpy(U, s->U.data(), s->U.size() * sizeof(s->U[0]));
+    return 0;
+  });
+}
+
+int oracle_set_primitive(void* hv, const void* V) {
+  Handle* h = static_cast<Handle*>(hv);
+  return dispatch(h, [&](auto* s) {
+    using Real = std::decay_t<decltype(s->gamma)>;
+    s->set_primitive(static_cast<const Real*>(V));
+    return 0;
+  });
+}
+
+int oracle_get_primitive(void* hv, void* V) {
+  Handle* h = static_cast<Handle*>(hv);
+  return dispatch(h, [&](auto* s) {
+    using Real = std::decay_t<decltype(s->gamma)>;
+    s->get_primitive(static_cast<Real*>(V));
     return 0;
   });
 }

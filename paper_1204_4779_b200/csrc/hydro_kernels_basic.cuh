@@ -104,6 +104,33 @@ __global__ void __launch_bounds__(256) k_cfl(const Real* __restrict__ U, Geom<Re
   block_reduce_and_finalize<Real>(s, bad, sc, g, gridDim.x, 0);
 }
 
+// ------------------------------------------------------------------ state_kind = primitive: conversions at the boundary
+// TO_CONS: V = (rho, v_a, p) -> U = (rho, rho v_a, E), E = fma(0.5 rho, q, p/(gamma-1)) (EOS PAPER.md:694, DESIGN.md §4
+// "cons"); otherwise U -> V by Eq. 19.  in == out is allowed (each thread touches only its own cell).
+template <class Real, int D, bool TO_CONS>
+__global__ void __launch_bounds__(256) k_convert(const Real* in, Real* out, Geom<Real> g) {
+  const long long c = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (c >= g.N) return;
+  Real a[D + 2], b[D + 2];
+  load_fields_rw<Real, D + 2>(in, g.N, c, a);
+  if (TO_CONS) {
+    Real q = a[1] * a[1];
+#pragma unroll
+    for (int d = 1; d < D; ++d) q = rfma(a[1 + d], a[1 + d], q);
+    b[0] = a[0];
+#pragma unroll
+    for (int d = 0; d < D; ++d) b[1 + d] = a[0] * a[1 + d];
+    b[D + 1] = rfma(Real(0.5) * a[0], q, a[D + 1] * g.igm1);
+  } else {
+    const Prim<Real, D> V = prim_of<Real, D>(a, g.gm1);
+    b[0] = V.rho;
+#pragma unroll
+    for (int d = 0; d < D; ++d) b[1 + d] = V.v[d];
+    b[D + 1] = V.p;
+  }
+  store_fields<Real, D + 2>(out, g.N, c, b);
+}
+
 // ------------------------------------------------------------------ manifest_all pieces
 // a1: V = V(U), Eq. 19
 template <class Real, int D>

@@ -49,6 +49,7 @@ struct paraiso_hydro {
   int boundary = BOUNDARY_PERIODIC, riemann = RIEMANN_HLLC, variant = VARIANT_FUSED;
   int block[3] = {0, 0, 0};
   int tile_depth = 0, cells_per_thread = 0, use_graph = 1;
+  int state_kind = 0;  // 0: set_state / get_state exchange conserved variables, 1: primitive variables
 
   void* U[2] = {nullptr, nullptr};  // U[0]: current state / U_base; U[1]: stage-1 result
   void* V = nullptr;                // manifest_all: primitives
@@ -277,6 +278,13 @@ struct Launch {
     h->launches += 1;
   }
 
+  template <bool TO_CONS>
+  static void convert(paraiso_hydro* h, const void* in, void* out) {
+    const int bs = 256;
+    k_convert<Real, D, TO_CONS><<<grid1d(h->N, bs), bs, 0, h->stream>>>((const Real*)in, (Real*)out, make_geom<Real>(h));
+    h->launches += 1;
+  }
+
   static void control(paraiso_hydro* h, int mode, double a, double b) {
     k_control<Real><<<1, 1, 0, h->stream>>>(h->sc, make_geom<Real>(h), mode, a, b);
     h->launches += 1;
@@ -411,7 +419,8 @@ static bool find_option(paraiso_hydro* h, const char* key, OptionRef* ref) {
                       {"block_z", {&h->block[2], 0, 64}},
                       {"tile_depth", {&h->tile_depth, 0, 1 << 20}},
                       {"cells_per_thread", {&h->cells_per_thread, 0, 8}},
-                      {"graph", {&h->use_graph, 0, 1}}};
+                      {"graph", {&h->use_graph, 0, 1}},
+                      {"state_kind", {&h->state_kind, 0, 1}}};
   for (const Opt& o : opts)
     if (!std::strcmp(key, o.key)) {
       *ref = o.ref;
@@ -450,6 +459,7 @@ int paraiso_hydro_set_state(paraiso_hydro_t* h, const void* U) {
   const size_t bytes = size_t(h->nf) * h->N * h->esize;
   CUDA_TRY(h, cudaMemcpyAsync(h->U[0], U, bytes, cudaMemcpyDefault, h->stream));
   dispatch(h, [&](auto L) {
+    if (h->state_kind == 1) L.template convert<true>(h, h->U[0], h->U[0]);
     L.control(h, CTRL_RESET, 0, 0);
     L.cfl(h);
   });
@@ -461,7 +471,12 @@ int paraiso_hydro_get_state(paraiso_hydro_t* h, void* U_out) {
   if (!h || !U_out) return fail(h, PARAISO_EINVAL, "get_state: null pointer");
   if (!h->has_state) return fail(h, PARAISO_ESTATE, "get_state: no state set");
   const size_t bytes = size_t(h->nf) * h->N * h->esize;
-  CUDA_TRY(h, cudaMemcpyAsync(U_out, h->U[0], bytes, cudaMemcpyDefault, h->stream));
+  const void* src = h->U[0];
+  if (h->state_kind == 1) {  // primitives are formed in the stage buffer, which is free between steps
+    dispatch(h, [&](auto L) { L.template convert<false>(h, h->U[0], h->U[1]); });
+    src = h->U[1];
+  }
+  CUDA_TRY(h, cudaMemcpyAsync(U_out, src, bytes, cudaMemcpyDefault, h->stream));
   cudaPointerAttributes at;
   cudaError_t e = cudaPointerGetAttributes(&at, U_out);
   if (e != cudaSuccess || at.type == cudaMemoryTypeUnregistered || at.type == cudaMemoryTypeHost) {

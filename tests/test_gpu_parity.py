@@ -240,3 +240,42 @@ def test_march_packed_needs_even_nx_and_falls_back(gpu, oracle_mod):
     assert np.array_equal(got, ref)
     got, _ = gpu_steps(gpu, w, 2, "march", cells_per_thread=2)  # explicit request: falls back to the first fused design
     assert np.array_equal(got, ref)
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("dims", [1, 2, 3])
+def test_state_kind_primitive_matches_oracle(gpu, oracle_mod, dims, dtype):
+    """Option state_kind = 1: set_state / get_state exchange primitive variables, converted on the device with the
+    arithmetic of DESIGN.md §4 ("cons", "prim"); compared with the oracle's conversion and a step in between."""
+    import torch
+
+    w = inputs.random_smooth(SHAPES[dims], dtype, seed=21 + dims)
+    o = oracle_mod.Oracle(w.n, w.extent, w.gamma, w.dtype, w.boundary, "hllc", "omp")
+    o.set_state(w.U)
+    V0 = o.get_primitive()
+    o.set_primitive(V0)
+    U0 = o.get_state()
+    dt = o.cfl_dt(w.cfl)
+    o.step(dt)
+    V1 = o.get_primitive()
+    o.close()
+    with gpu.ParaisoHydro(w.n, w.extent, w.gamma, w.dtype, w.boundary, "hllc", state_kind=1) as h:
+        h.set_state(torch.from_numpy(V0).cuda())
+        gdt = h.cfl_dt(w.cfl)
+        assert abs(gdt - dt) <= TOL[np.dtype(dtype)][2] * dt
+        assert np.array_equal(h.get_state(), o_prim_roundtrip(oracle_mod, w, U0))  # conserved -> primitive, no step
+        h.set_option("state_kind", 0)
+        assert np.array_equal(h.get_state(), U0)                                   # what set_state stored
+        h.set_option("state_kind", 1)
+        h.step(gdt)
+        got = h.get_state()
+        assert h.stats() == 0
+    assert np.array_equal(got, V1)
+
+
+def o_prim_roundtrip(oracle_mod, w, U):
+    o = oracle_mod.Oracle(w.n, w.extent, w.gamma, w.dtype, w.boundary)
+    o.set_state(U)
+    V = o.get_primitive()
+    o.close()
+    return V

@@ -362,3 +362,40 @@ def test_omp_build_is_bit_identical_to_serial(oracle_mod):
     kb = b.run(0.3, 7)
     assert ka == kb
     assert np.array_equal(a.get_state(), b.get_state())
+
+
+# ---------------------------------------------------------------- P13
+def test_p13_primitive_conserved_conversion(oracle_mod):
+    """EOS PAPER.md:694, E = p/(gamma-1) + rho v^2/2, and Eq. 19 its inverse.  Closed forms chosen so that every
+    intermediate is exact in binary: a dropped kinetic term, a missing 1/2, gamma instead of gamma-1 or a swapped
+    component all change them."""
+    # gamma = 1.5 -> 1/(gamma-1) = 2 exactly
+    n, ext = (4, 4, 4), (1.0, 1.0, 1.0)
+    V = np.zeros((5,) + n)
+    V[0], V[1], V[2], V[3], V[4] = 2.0, 3.0, -1.0, 0.5, 0.75
+    for dtype in (np.float32, np.float64):
+        o = oracle_mod.Oracle(n, ext, 1.5, dtype)
+        o.set_primitive(V)
+        U = o.get_state()
+        # m = rho v = (6, -2, 1); q = 9 + 1 + 0.25 = 10.25; E = 0.75 * 2 + 0.5 * 2 * 10.25 = 11.75
+        assert np.all(U[0] == 2.0) and np.all(U[1] == 6.0) and np.all(U[2] == -2.0) and np.all(U[3] == 1.0)
+        assert np.all(U[4] == 11.75)
+        assert np.array_equal(o.get_primitive(), V.astype(dtype))  # exact round trip on exact data
+        o.close()
+    # 1-D and 2-D use only their own velocity components
+    o = oracle_mod.Oracle((8,), (1.0,), 1.5, np.float64)
+    o.set_primitive(np.stack([np.full(8, 2.0), np.full(8, 3.0), np.full(8, 0.75)]))
+    assert np.all(o.get_state()[2] == 0.75 * 2 + 9.0)
+    o.close()
+    # generic data: agreement with the fp64 conversion the input generators use, and the round trip to rounding
+    w = inputs.random_smooth((12, 10, 6), np.float64, seed=9)
+    o = oracle_mod.Oracle(w.n, w.extent, w.gamma, np.float64)
+    o.set_state(w.U)
+    P = o.get_primitive()
+    assert P[0].min() > 0 and P[4].min() > 0
+    o.set_primitive(P)
+    back = o.get_state()
+    assert np.max(np.abs(back - w.U) / np.abs(w.U).max()) < 4e-16
+    ref = numpy_scheme.prim(w.U, w.gamma)
+    assert np.max(np.abs(P - ref)) < 1e-14
+    o.close()
