@@ -43,7 +43,7 @@ def _lib(kind="serial"):
 class Oracle:
     """One oracle solver instance.  State arrays are (nf, [nz,] [ny,] nx), x fastest."""
 
-    def __init__(self, n, extent, gamma, dtype, boundary="periodic", riemann="hllc", threads="serial"):
+    def __init__(self, n, extent, gamma, dtype, boundary="periodic", riemann="hllc", threads="serial", integrator="midpoint"):
         self.n = tuple(int(v) for v in n)  # x first
         self.dims = len(self.n)
         self.dtype = np.dtype(dtype)
@@ -57,6 +57,7 @@ class Oracle:
             raise ValueError("oracle_create failed")
         self._opt("boundary", {"periodic": 0, "outflow": 1}[boundary])
         self._opt("riemann", {"hllc": 0, "hll": 1}[riemann])
+        self._opt("integrator", {"midpoint": 0, "heun": 1}[integrator])
 
     def _opt(self, key, val):
         if self._L.oracle_set_option(self._h, key.encode(), val) != 0:

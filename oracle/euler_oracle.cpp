@@ -274,11 +274,20 @@ struct Solver {
     }
   }
 
-  // Eq. 24-27 (midpoint form, R7).
+  // Eq. 24-27 (midpoint form, R7) -- the paper's integrator, the default.
+  // integrator = 1: the two-stage TVD Runge-Kutta scheme north_star names as the fallback (Heun / Shu-Osher
+  // SSP-RK2, R20):  U1 = U0 + dt L(U0);  U2 = 0.5 (U0 + (U1 + dt L(U1))).  An option, never the default.
+  int integrator = 0;
   void step(Real dt) {
     std::vector<Real> U1, U2;
-    stage(U, U, Real(0.5) * dt, U1);
-    stage(U1, U, dt, U2);
+    if (integrator == 0) {
+      stage(U, U, Real(0.5) * dt, U1);
+      stage(U1, U, dt, U2);
+    } else {
+      stage(U, U, dt, U1);
+      stage(U1, U1, dt, U2);
+      for (size_t i = 0; i < U2.size(); ++i) U2[i] = Real(0.5) * (U[i] + U2[i]);
+    }
     U.swap(U2);
   }
 
@@ -375,6 +384,10 @@ int oracle_set_option(void* hv, const char* key, int64_t value) {
     }
     if (!std::strcmp(key, "riemann") && (value == 0 || value == 1)) {
       s->riemann_kind = int(value);
+      return 0;
+    }
+    if (!std::strcmp(key, "integrator") && (value == 0 || value == 1)) {
+      s->integrator = int(value);
       return 0;
     }
     return -1;

@@ -48,7 +48,7 @@ __device__ __forceinline__ double bits_real<double>(unsigned long long b) {
 template <class Real>
 __device__ __forceinline__ void set_lambdas(Scalars* sc, Real dt, const Geom<Real>& g) {
   sc->dt = double(dt);
-  const Real tau1 = Real(0.5) * dt;
+  const Real tau1 = g.integrator == 1 ? dt : Real(0.5) * dt;  // Heun: both stages advance by dt
 #pragma unroll
   for (int a = 0; a < 3; ++a) {
     sc->lam[0][a] = double(rdiv(tau1, g.dr[a]));

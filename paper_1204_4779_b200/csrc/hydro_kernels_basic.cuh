@@ -261,6 +261,12 @@ __global__ void __launch_bounds__(256) k_update(const Real* Ubase, Real* Uout,
     add_axis<Real, D, 0>(u, fa, g, c, idx, Real(sc->lam[STAGE - 1][0]));
     if constexpr (D > 1) add_axis<Real, D, 1>(u, fa, g, c, idx, Real(sc->lam[STAGE - 1][1]));
     if constexpr (D > 2) add_axis<Real, D, 2>(u, fa, g, c, idx, Real(sc->lam[STAGE - 1][2]));
+    if (STAGE == 2 && g.integrator == 1) {  // Heun: U2 = 0.5 (U0 + (U1 + dt L(U1))); U0 still sits in Uout
+      Real u0[D + 2];
+      load_fields_rw<Real, D + 2>(Uout, g.N, c, u0);
+#pragma unroll
+      for (int f = 0; f < D + 2; ++f) u[f] = Real(0.5) * (u0[f] + u[f]);
+    }
     store_fields<Real, D + 2>(Uout, g.N, c, u);
     if (STAGE == 2) {
       Real ir;
@@ -298,6 +304,12 @@ __global__ void __launch_bounds__(128) k_delayed(const Real* __restrict__ Uin, c
     delayed_axis<Real, D, 0, RS>(u, Uin, g, c, idx, Real(sc->lam[STAGE - 1][0]));
     if constexpr (D > 1) delayed_axis<Real, D, 1, RS>(u, Uin, g, c, idx, Real(sc->lam[STAGE - 1][1]));
     if constexpr (D > 2) delayed_axis<Real, D, 2, RS>(u, Uin, g, c, idx, Real(sc->lam[STAGE - 1][2]));
+    if (STAGE == 2 && g.integrator == 1) {  // Heun: U2 = 0.5 (U0 + (U1 + dt L(U1))); U0 still sits in Uout
+      Real u0[D + 2];
+      load_fields_rw<Real, D + 2>(Uout, g.N, c, u0);
+#pragma unroll
+      for (int f = 0; f < D + 2; ++f) u[f] = Real(0.5) * (u0[f] + u[f]);
+    }
     store_fields<Real, D + 2>(Uout, g.N, c, u);
     if (STAGE == 2) {
       Real ir;

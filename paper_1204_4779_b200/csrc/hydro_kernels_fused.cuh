@@ -284,6 +284,12 @@ __global__ void __launch_bounds__(TX* TY)
 #pragma unroll
         for (int f = 0; f < NF; ++f) u[f] = rfma(lam1, Fprev[f] - Fnext[f], u[f]);
       }
+      if (STAGE == 2 && g.integrator == 1) {  // Heun: U2 = 0.5 (U0 + (U1 + dt L(U1))); U0 still sits in Uout
+        Real u0[NF];
+        load_fields_rw<Real, NF>(Uout, N, plane_of(m) + own, u0);
+#pragma unroll
+        for (int f = 0; f < NF; ++f) u[f] = Real(0.5) * (u0[f] + u[f]);
+      }
       store_fields<Real, NF>(Uout, N, plane_of(m) + own, u);
       if (STAGE == 2) {
         Real ir;

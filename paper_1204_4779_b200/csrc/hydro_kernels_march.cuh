@@ -364,6 +364,10 @@ __global__ void __launch_bounds__(MarchShape<T, D, NWX, TY>::NT, MINB)
 #pragma unroll
             for (int f = 0; f < NF; ++f) u[f] = rfma(lam1, Fprev[f] - Fnext[f], u[f]);
           }
+          if (STAGE == 2 && g.integrator == 1) {  // Heun: U2 = 0.5 (U0 + (U1 + dt L(U1))); U0 still sits in Uout
+#pragma unroll
+            for (int f = 0; f < NF; ++f) u[f] = S(0.5) * (ld_cells_rw<T>(Uout, f * Ni + cell) + u[f]);
+          }
 #pragma unroll
           for (int f = 0; f < NF; ++f) st_cells<T>(Uout, f * Ni + cell, u[f]);
           if (STAGE == 2) {
@@ -582,7 +586,7 @@ bool launch_march_stage(const Real* Uin, const Real* Ubase, Real* Uout, const Ge
       if (packed) return launch_march_shape<f32x2, D, RS, STAGE, NWXV, 1, 1>(Uin, Ubase, Uout, g, sc, stream, depth); \
     return launch_march_shape<Real, D, RS, STAGE, NWXV, 1, minb>(Uin, Ubase, Uout, g, sc, stream, depth);           \
   }
-      PH_SHAPE(2) PH_SHAPE(4) PH_SHAPE(8)
+      PH_SHAPE(2) PH_SHAPE(3) PH_SHAPE(4) PH_SHAPE(7) PH_SHAPE(8)
 #undef PH_SHAPE
       return false;
     } else {

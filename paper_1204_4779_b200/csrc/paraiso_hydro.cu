@@ -49,6 +49,7 @@ struct paraiso_hydro {
   int boundary = BOUNDARY_PERIODIC, riemann = RIEMANN_HLLC, variant = VARIANT_FUSED;
   int block[3] = {0, 0, 0};
   int tile_depth = 0, cells_per_thread = 0, use_graph = 1;
+  int integrator = 0;  // 0 midpoint (paper) | 1 Heun
   int state_kind = 0;  // 0: set_state / get_state exchange conserved variables, 1: primitive variables
 
   void* U[2] = {nullptr, nullptr};  // U[0]: current state / U_base; U[1]: stage-1 result
@@ -107,6 +108,7 @@ static Geom<Real> make_geom(const paraiso_hydro* h) {
   g.gm1 = g.gamma - Real(1);
   g.igm1 = Real(1) / g.gm1;
   g.boundary = h->boundary;
+  g.integrator = h->integrator;
   return g;
 }
 
@@ -181,6 +183,11 @@ static int ensure_intermediates(paraiso_hydro* h) {
 template <class Real, int D, int RS>
 struct Launch {
   static unsigned int grid1d(int64_t N, int bs) { return (unsigned int)((N + bs - 1) / bs); }
+  // U_base of Eq. 23: U0 in both stages of the midpoint rule; Heun's second stage starts from U1
+  template <int STAGE>
+  static const Real* stage_base(const paraiso_hydro* h) {
+    return (const Real*)((STAGE == 2 && h->integrator == 1) ? h->U[1] : h->U[0]);
+  }
 
   template <int A>
   static void recon_riemann(paraiso_hydro* h, const Geom<Real>& g) {
@@ -206,7 +213,7 @@ struct Launch {
       fa.Fb[a] = (const Real*)h->Fb[a];
     }
     const int bs = 256;
-    k_update<Real, D, STAGE><<<grid1d(h->N, bs), bs, 0, h->stream>>>((const Real*)h->U[0], Uout, fa, g, h->sc);
+    k_update<Real, D, STAGE><<<grid1d(h->N, bs), bs, 0, h->stream>>>(stage_base<STAGE>(h), Uout, fa, g, h->sc);
     h->launches += 1;
   }
 
@@ -243,14 +250,14 @@ struct Launch {
       case VARIANT_FUSED:  // the faster of the two on-chip designs per grid kind: 3-D k_march, 2-D k_fused
       case VARIANT_MARCH:
         if ((h->variant == VARIANT_MARCH || D == 3) &&
-            launch_march_stage<Real, D, RS, STAGE>(Uin, (const Real*)h->U[0], Uout, g, h->sc, h->stream, h->block,
+            launch_march_stage<Real, D, RS, STAGE>(Uin, stage_base<STAGE>(h), Uout, g, h->sc, h->stream, h->block,
                                                    h->tile_depth, h->cells_per_thread)) {
           h->launches += 1;
           break;
         }
         // shapes the marching kernel does not cover: the first fused design
       case VARIANT_FUSED1:
-        if (launch_fused_stage<Real, D, RS, STAGE>(Uin, (const Real*)h->U[0], Uout, g, h->sc, h->stream, h->block,
+        if (launch_fused_stage<Real, D, RS, STAGE>(Uin, stage_base<STAGE>(h), Uout, g, h->sc, h->stream, h->block,
                                                    h->tile_depth)) {
           h->launches += 1;
           break;
@@ -258,7 +265,7 @@ struct Launch {
         // 1-D grids (and shapes the marching kernel does not cover) use the Delayed kernel: fall through
       default: {
         const int bs = h->block[0] > 0 ? h->block[0] : 128;
-        k_delayed<Real, D, RS, STAGE><<<grid1d(h->N, bs), bs, 0, h->stream>>>(Uin, (const Real*)h->U[0], Uout, g, h->sc);
+        k_delayed<Real, D, RS, STAGE><<<grid1d(h->N, bs), bs, 0, h->stream>>>(Uin, stage_base<STAGE>(h), Uout, g, h->sc);
         h->launches += 1;
       }
     }
@@ -326,7 +333,7 @@ static int check_launch(paraiso_hydro* h) {
 }
 
 static int options_key(const paraiso_hydro* h) {
-  int k = h->boundary | (h->riemann << 1) | (h->variant << 2);
+  int k = h->boundary | (h->riemann << 1) | (h->integrator << 2) | (h->variant << 3);
   k = k * 1031 + h->block[0];
   k = k * 1031 + h->block[1];
   k = k * 1031 + h->block[2];
@@ -420,7 +427,8 @@ static bool find_option(paraiso_hydro* h, const char* key, OptionRef* ref) {
                       {"tile_depth", {&h->tile_depth, 0, 1 << 20}},
                       {"cells_per_thread", {&h->cells_per_thread, 0, 8}},
                       {"graph", {&h->use_graph, 0, 1}},
-                      {"state_kind", {&h->state_kind, 0, 1}}};
+                      {"state_kind", {&h->state_kind, 0, 1}},
+                      {"integrator", {&h->integrator, 0, 1}}};
   for (const Opt& o : opts)
     if (!std::strcmp(key, o.key)) {
       *ref = o.ref;

@@ -279,3 +279,42 @@ def o_prim_roundtrip(oracle_mod, w, U):
     V = o.get_primitive()
     o.close()
     return V
+
+
+@pytest.mark.parametrize("variant", ["fused", "march", "fused1"])
+@pytest.mark.parametrize("n", [(4, 301), (513, 4), (4, 5, 130), (130, 4, 4), (4, 67, 4)])
+def test_extreme_aspect_grids(gpu, oracle_mod, variant, n):
+    """One axis at the legal minimum, another spanning many tiles: every tile is mostly halo, every halo wraps."""
+    for boundary in ("periodic", "outflow"):
+        w = inputs.random_smooth(n, np.float32, seed=17, boundary=boundary)
+        ref, _ = oracle_steps(oracle_mod, w, 3)
+        got, _ = gpu_steps(gpu, w, 3, variant)
+        assert np.all(field_errors(got, ref) <= 3e-5), (n, boundary)
+        assert np.array_equal(got, ref), (n, boundary)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("dims", [1, 2, 3])
+def test_heun_integrator_option_matches_oracle(gpu, oracle_mod, variant, dims, dtype):
+    """Option integrator = 1 (Heun / SSP-RK2, R20), stepped by hand and device-paced (graph replay)."""
+    import torch
+
+    w = inputs.random_smooth(SHAPES[dims], dtype, seed=31 + dims)
+    o = oracle_mod.Oracle(w.n, w.extent, w.gamma, w.dtype, w.boundary, "hllc", "omp", "heun")
+    o.set_state(w.U)
+    k, t = o.run(w.cfl, 11)
+    ref = o.get_state()
+    o.close()
+    tol1 = TOL[np.dtype(dtype)][0]
+    with gpu.ParaisoHydro(w.n, w.extent, w.gamma, w.dtype, w.boundary, "hllc", variant, integrator=1) as h:
+        h.set_state(torch.from_numpy(w.U).cuda())
+        for _ in range(2):
+            h.step(h.cfl_dt(w.cfl))
+        h.run(w.cfl, 9)  # 8 steps from the captured graph + 1 plain
+        got = h.get_state()
+        tg, kg = h.time()
+        assert h.stats() == 0 and kg == 11
+    assert abs(tg - t) <= 20 * TOL[np.dtype(dtype)][2] * t
+    assert np.all(field_errors(got, ref) <= 11 * tol1), field_errors(got, ref)
+    assert np.array_equal(got, ref)

@@ -399,3 +399,59 @@ def test_p13_primitive_conserved_conversion(oracle_mod):
     ref = numpy_scheme.prim(w.U, w.gamma)
     assert np.max(np.abs(P - ref)) < 1e-14
     o.close()
+
+
+# ---------------------------------------------------------------- P14 (option integrator = heun, R20)
+@pytest.mark.parametrize("boundary", ["periodic", "outflow"])
+@pytest.mark.parametrize("n", [(8,), (6, 5), (5, 4, 6)])
+def test_p14_heun_matches_its_definition_in_numpy(oracle_mod, n, boundary):
+    """U1 = U0 + dt L(U0); U2 = (U0 + U1 + dt L(U1)) / 2, assembled here from the independent NumPy stage of P11."""
+    w = inputs.random_smooth(n, np.float64, seed=8, boundary=boundary)
+    o = oracle_mod.Oracle(w.n, w.extent, w.gamma, w.dtype, boundary, "hllc", "serial", "heun")
+    o.set_state(w.U)
+    dr = [e / m for e, m in zip(w.extent, w.n)]
+    U = w.U.astype(np.float64)
+    for _ in range(3):
+        dt = o.cfl_dt(0.4)
+        o.step(dt)
+        U1 = numpy_scheme.stage(U, U, dt, dr, w.gamma, boundary, "hllc")
+        U = 0.5 * (U + numpy_scheme.stage(U1, U1, dt, dr, w.gamma, boundary, "hllc"))
+        got = o.get_state()
+        for f in range(w.nf):
+            assert np.max(np.abs(got[f] - U[f])) <= 1e-13 * max(1.0, np.abs(U[f]).max())
+    # not the midpoint rule: the two integrators differ at third order in dt, visibly on this coarse grid
+    m = make(oracle_mod, w, boundary=boundary)
+    for _ in range(3):
+        m.step(m.cfl_dt(0.4))
+    d = np.abs(m.get_state() - got).max()
+    assert 1e-9 < d < 0.5, d
+
+
+def test_p14_heun_invariants_and_order(oracle_mod):
+    # a uniform state is a bitwise fixed point (0.5 * (U + U) = U exactly), mass / momentum / energy are conserved
+    U0 = uniform_state((9, 7), np.float32, (0.3, -0.2))
+    o = oracle_mod.Oracle((9, 7), (1.0, 1.0), 1.4, np.float32, "periodic", "hllc", "serial", "heun")
+    o.set_state(U0)
+    o.run(0.4, 20)
+    assert np.array_equal(o.get_state(), U0)
+    w = inputs.random_smooth((24, 16), np.float64, seed=5)
+    o = oracle_mod.Oracle(w.n, w.extent, w.gamma, w.dtype, "periodic", "hllc", "serial", "heun")
+    o.set_state(w.U)
+    s0 = [math.fsum(f.ravel()) for f in w.U]
+    scale = [math.fsum(np.abs(f.ravel())) for f in w.U]
+    o.run(0.4, 50)
+    U = o.get_state()
+    for f in range(w.nf):
+        assert abs(math.fsum(U[f].ravel()) - s0[f]) / scale[f] < 1e-14
+    # second order on the paper's entropy wave (Eq. 28), like the midpoint rule (P6)
+    def l1(n):
+        x = (np.arange(n) + 0.5) / n
+        rho = 2.0 + np.sin(2 * np.pi * x)
+        o = oracle_mod.Oracle((n,), (1.0,), 1.4, np.float64, "periodic", "hllc", "serial", "heun")
+        o.set_state(inputs.conserved_from_primitive(rho, [np.ones(n)], np.ones(n), 1.4))
+        _, t = o.run(0.4, 10**7, 1.0)
+        assert t == 1.0
+        return np.abs(o.get_state()[0] - rho).mean()
+    e = [l1(n) for n in (64, 128, 256)]
+    orders = [math.log2(a / b) for a, b in zip(e, e[1:])]
+    assert orders[0] > 1.5 and orders[1] > 1.7 and orders[1] < 2.2, orders
