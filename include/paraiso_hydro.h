@@ -71,6 +71,8 @@ int paraiso_hydro_destroy(paraiso_hydro_t *h);
  *               3 delayed     one kernel per stage, every thread recomputes all it needs from U
  *   "block_x" "block_y" "block_z" "tile_depth" "cells_per_thread"   launch-shape knobs of the sweep (0 = default)
  *   "graph"     1 replay steps of run() from a captured CUDA graph (default) | 0 plain launches
+ *   "staging"   k_march only: 0 / 1 every thread loads its own cells (default) | 2 TMA bulk copies of the tile rows into a
+ *               shared-memory ring (one cell per thread, n_x a multiple of 16 bytes; measured slower)
  *   "integrator" 0 the paper's two-stage midpoint rule, Eq. 24-27 (default) | 1 Heun / Shu-Osher SSP-RK2, the
  *               "2-stage TVD Runge-Kutta" north_star names as the fallback (R20): same kernels and traffic
  *   "state_kind" 0 set_state / get_state exchange conserved variables U = (rho, m_a, E) (default) |

@@ -79,7 +79,7 @@ __device__ __forceinline__ int bad_lanes(const Prim<T, D>& V, T E) {
   return lane_count(m_or(m_or(m_not(gt(V.rho, zero)), m_not(gt(V.p, zero))), m_not(le(rabs(E), T(S(3.0e38))))));
 }
 
-template <class T, int D, int NWX, int TY>
+template <class T, int D, int NWX, int TY, bool TMA = false>
 struct MarchShape {
   using S = scalar_t<T>;
   static constexpr int W = LaneTraits<T>::W;
@@ -101,7 +101,14 @@ struct MarchShape {
   static constexpr bool YH_MAIN = false;
   static_assert(D == 2 || !YH_MAIN || TY >= 4, "four different main warps fill the y halo rows");
   static_assert(XTASK_LANES <= 32, "tile too tall for one halo warp");
+  static constexpr int RING = 4;                        // TMA: raw planes m .. m+3 of the tile's own cells
   struct Smem {
+    // TMA staging (bulk async copies, one per tile row and field, complete on an mbarrier): the conserved state of
+    // the tile's own cells, planes m .. m+3 of U_in (stage 1 takes U_base from the same ring) and, for the last
+    // stage, planes m, m+1 of U_base = U0.  Rows are 16-byte aligned: first members of a 128-byte aligned struct.
+    S Uraw[TMA ? RING : 1][TMA ? NF : 1][TMA ? XROWS : 1][TMA ? TXC : 4];
+    S Ub[TMA ? 2 : 1][TMA ? NF : 1][TMA ? XROWS : 1][TMA ? TXC : 4];
+    unsigned long long mbar[RING + 2];
     S V[2][NF][PY][PX];                                 // primitives of plane m (double-buffered), halo 2
     S LOy[(D == 3) ? NF : 1][TY + 1][(D == 3) ? TXC : 2];  // [r]: low-side y state of tile row r (r = TY: halo warp)
     S Fy[(D == 3) ? NF : 1][TY][(D == 3) ? TXC : 2];    // [r]: flux through the low y face of tile row r (r = 0: halo warp)
@@ -167,24 +174,52 @@ __device__ __forceinline__ double shfl_up(double v) { return __shfl_up_sync(0xff
 
 // All warps of the block arrive at barrier 0 the same number of times, the main warps and the halo warp from
 // different places in the code (PTX bar.sync semantics: arrival is counted per warp, not per call site).
+// ---------------------------------------------------------------- TMA bulk copies completing on an mbarrier
+__device__ __forceinline__ unsigned int smem_addr(const void* p) { return (unsigned int)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_addr(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, int bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_addr(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned int parity) {
+  unsigned int done;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(done)
+        : "r"(smem_addr(bar)), "r"(parity)
+        : "memory");
+  } while (!done);
+}
+// global -> shared, `bytes` a multiple of 16, both addresses 16-byte aligned (cp.async.bulk: SASS UBLKCP)
+__device__ __forceinline__ void tma_row(void* dst, const void* src, int bytes, unsigned long long* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_addr(dst)),
+               "l"(src), "r"(bytes), "r"(smem_addr(bar))
+               : "memory");
+}
+
 #ifdef PH_EXPERIMENT_NO_BARRIER  // timing ablation of profiles/r1c_README.md (racy, wrong results); never defined by build.py
 __device__ __forceinline__ void block_barrier() { __syncwarp(); }
 #else
 __device__ __forceinline__ void block_barrier() { asm volatile("bar.sync 0;" ::: "memory"); }
 #endif
 
-template <class T, int D, int RS, int STAGE, int NWX, int TY, int MINB>
-__global__ void __launch_bounds__(MarchShape<T, D, NWX, TY>::NT, MINB)
+template <class T, int D, int RS, int STAGE, int NWX, int TY, int MINB, bool TMA>
+__global__ void __launch_bounds__(MarchShape<T, D, NWX, TY, TMA>::NT, MINB)
     k_march(const scalar_t<T>* __restrict__ Uin, const scalar_t<T>* Ubase, scalar_t<T>* Uout, Geom<scalar_t<T>> g,
             Scalars* sc, int depth) {
-  using Sh = MarchShape<T, D, NWX, TY>;
+  using Sh = MarchShape<T, D, NWX, TY, TMA>;
   using S = scalar_t<T>;
   using P = Prim<T, D>;
   constexpr int W = Sh::W, NF = Sh::NF, TXC = Sh::TXC, OY = Sh::OY, XROWS = Sh::XROWS;
   constexpr int M = D - 1;  // marching axis
+  constexpr int RING = Sh::RING;
 
   if (sc->done) return;
-  extern __shared__ __align__(16) unsigned char march_smem_raw[];
+  extern __shared__ __align__(128) unsigned char march_smem_raw[];
   typename Sh::Smem& sm = *reinterpret_cast<typename Sh::Smem*>(march_smem_raw);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -198,6 +233,9 @@ __global__ void __launch_bounds__(MarchShape<T, D, NWX, TY>::NT, MINB)
   const int psi = (D == 3) ? nx * ny : nx;              // cells per plane
   auto plane_of = [&](int m) { return map_index(m, nM, bnd) * psi; };
   auto grid_row = [&](int gj) { return (D == 3) ? march_src(gj, ny, bnd) * nx : 0; };
+
+  // TMA staging needs whole, 16-byte aligned rows: tiles that end inside the grid (the launcher checks n_x % 4)
+  const bool use_tma = TMA && (x0 + TXC <= nx);
 
   S s_max = S(0);
   int bad = 0;
@@ -246,7 +284,7 @@ __global__ void __launch_bounds__(MarchShape<T, D, NWX, TY>::NT, MINB)
       Vc = prim_of<T, D>(u, g.gm1);
       load_cells_of(src, m0 + 1, u);
       Vp1 = prim_of<T, D>(u, g.gm1);
-      load_cells_of(src, m0 + 2, Unext);
+      if (!use_tma) load_cells_of(src, m0 + 2, Unext);
       P him1, loc;
       interpolate<T, D>(Vm2, Vm1, Vc, nullptr, &him1);
       interpolate<T, D>(Vm1, Vc, Vp1, &loc, &hiM);
@@ -295,8 +333,14 @@ __global__ void __launch_bounds__(MarchShape<T, D, NWX, TY>::NT, MINB)
         for (int f = 0; f < NF; ++f) sts(&sm.LOy[f][row][c0], a[f]);
       }
       // marching axis: V[m+2], slope of cell m+1, flux through face m+1/2
+      const int q = m - m0;  // plane index inside this block's march
+      if (TMA && use_tma) {  // U_in of plane m+2: landed in ring slot (q+2) % RING one iteration ago
+        mbar_wait(&sm.mbar[(q + 2) % RING], ((q + 2) / RING) & 1);
+#pragma unroll
+        for (int f = 0; f < NF; ++f) Unext[f] = lds<T>(&sm.Uraw[(q + 2) % RING][f][row][c0]);
+      }
       const P Vp2 = prim_of<T, D>(Unext, g.gm1);
-      if (more) load_cells_of(src, m + 3, Unext);
+      if (more && !use_tma) load_cells_of(src, m + 3, Unext);
       P loM1, hiM1;
       interpolate<T, D>(Vc, Vp1, Vp2, &loM1, &hiM1);
       T Fnext[NF];
@@ -336,7 +380,17 @@ __global__ void __launch_bounds__(MarchShape<T, D, NWX, TY>::NT, MINB)
       // own-cell base state of Eq. 23 (coherent load: the last stage overwrites U_base in place)
       const int cell = plane_of(m) + own;
       T u[NF];
-      if (active) {
+      if (TMA && use_tma) {  // stage 1: U_base = U_in, plane m of the ring; last stage: the U0 ring
+        if (STAGE == 1) {
+          mbar_wait(&sm.mbar[q % RING], (q / RING) & 1);
+#pragma unroll
+          for (int f = 0; f < NF; ++f) u[f] = lds<T>(&sm.Uraw[q % RING][f][row][c0]);
+        } else {
+          mbar_wait(&sm.mbar[RING + (q & 1)], (q >> 1) & 1);
+#pragma unroll
+          for (int f = 0; f < NF; ++f) u[f] = lds<T>(&sm.Ub[q & 1][f][row][c0]);
+        }
+      } else if (active) {
 #pragma unroll
         for (int f = 0; f < NF; ++f) u[f] = ld_cells_rw<T>(Ubase, f * Ni + cell);
       }
@@ -462,6 +516,35 @@ __global__ void __launch_bounds__(MarchShape<T, D, NWX, TY>::NT, MINB)
       return prim_from_fields<T, D>(u);
     };
 
+    // TMA producer: one bulk copy per field and tile row (jobs spread over the lanes), completing on the slot's mbarrier
+    constexpr int NJOB = NF * XROWS, JPL = (NJOB + 31) / 32;
+    constexpr int ROW_BYTES = TXC * (int)sizeof(S);
+    int job_off[JPL];  // element offset of the row inside a plane + f * N
+#pragma unroll
+    for (int j = 0; j < JPL; ++j) {
+      const int job = lane + 32 * j;
+      const int f = job / XROWS, r = job - f * XROWS;
+      job_off[j] = job < NJOB ? f * Ni + grid_row(y0 + r) + x0 : -1;
+    }
+    auto tma_plane = [&](const S* A, int m, S* dst_slot, unsigned long long* bar) {
+      const int pl = plane_of(m);
+      if (lane == 0) mbar_expect_tx(bar, NJOB * ROW_BYTES);
+      __syncwarp();
+#pragma unroll
+      for (int j = 0; j < JPL; ++j)
+        if (job_off[j] >= 0) tma_row(dst_slot + (size_t)(lane + 32 * j) * TXC, A + (job_off[j] + pl), ROW_BYTES, bar);
+    };
+    if (TMA && use_tma) {
+      if (lane == 0) {
+#pragma unroll
+        for (int i = 0; i < RING + 2; ++i) mbar_init(&sm.mbar[i], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+      }
+      __syncwarp();
+#pragma unroll
+      for (int k = 0; k < 3; ++k) tma_plane(Uin, m0 + k, &sm.Uraw[k][0][0][0], &sm.mbar[k]);
+      if (STAGE == 2) tma_plane(Ubase, m0, &sm.Ub[0][0][0][0], &sm.mbar[RING]);
+    }
     load_halo(m0);
     store_halo(0);
     block_barrier();
@@ -470,6 +553,11 @@ __global__ void __launch_bounds__(MarchShape<T, D, NWX, TY>::NT, MINB)
     for (int m = m0; m < m1; ++m, b ^= 1) {
       const bool more = m + 1 < m1;
       // ---- phase A: high-side states of the cells just below the tile, low-side states of those just above
+      if (TMA && use_tma && more) {  // every reader of the slots written here passed the last block barrier
+        const int q = m - m0;
+        tma_plane(Uin, m + 3, &sm.Uraw[(q + 3) % RING][0][0][0], &sm.mbar[(q + 3) % RING]);
+        if (STAGE == 2) tma_plane(Ubase, m + 1, &sm.Ub[(q + 1) & 1][0][0][0], &sm.mbar[RING + ((q + 1) & 1)]);
+      }
       if (more) load_halo(m + 1);
       P hiYlow, hiXlow;
       if constexpr (D == 3) {
@@ -526,11 +614,11 @@ __global__ void __launch_bounds__(MarchShape<T, D, NWX, TY>::NT, MINB)
 }
 
 // ------------------------------------------------------------------------------------------------
-template <class T, int D, int RS, int STAGE, int NWX, int TY, int MINB>
+template <class T, int D, int RS, int STAGE, int NWX, int TY, int MINB, bool TMA = false>
 static bool launch_march_shape(const scalar_t<T>* Uin, const scalar_t<T>* Ubase, scalar_t<T>* Uout,
                                const Geom<scalar_t<T>>& g, Scalars* sc, cudaStream_t stream, int depth) {
-  using Sh = MarchShape<T, D, NWX, TY>;
-  auto kern = k_march<T, D, RS, STAGE, NWX, TY, MINB>;
+  using Sh = MarchShape<T, D, NWX, TY, TMA>;
+  auto kern = k_march<T, D, RS, STAGE, NWX, TY, MINB, TMA>;
   static bool configured = false;
   if (!configured) {
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(typename Sh::Smem)) != cudaSuccess)
@@ -565,9 +653,11 @@ inline int march_default_depth(long long tiles_in_plane, int nM) {
 //   pack: cells per thread along x (0 = default = 1; 2 = packed f32x2, fp32 on an even n_x only: measured slower,
 //         DESIGN.md §7)
 //   block[0] (2-D): main warps per block (0 = default); block[1] (3-D): tile rows TY (0 = default)
+//   staging: 0 / 1 = every thread loads its own cells (LDG), 2 = TMA bulk copies of the tile rows into a shared-memory
+//            ring (one cell per thread, n_x a multiple of 16 bytes, default tile shapes only)
 template <class Real, int D, int RS, int STAGE>
 bool launch_march_stage(const Real* Uin, const Real* Ubase, Real* Uout, const Geom<Real>& g, Scalars* sc,
-                        cudaStream_t stream, const int* block, int tile_depth, int pack) {
+                        cudaStream_t stream, const int* block, int tile_depth, int pack, int staging) {
   if constexpr (D == 1) {
     return false;
   } else {
@@ -576,6 +666,7 @@ bool launch_march_stage(const Real* Uin, const Real* Ubase, Real* Uout, const Ge
     const bool packed = can_pack && pack == 2 && (g.n[0] % 2 == 0);
     if (pack == 2 && !packed) return false;
     const int w = packed ? 2 : 1;
+    const bool tma = staging == 2 && !packed && g.n[0] % (16 / (int)sizeof(Real)) == 0;
     if constexpr (D == 2) {
       int nwx = block[0] > 0 ? block[0] : 4;
       const long long tiles = (g.n[0] + nwx * 32 * w - 1) / (nwx * 32 * w);
@@ -586,6 +677,7 @@ bool launch_march_stage(const Real* Uin, const Real* Ubase, Real* Uout, const Ge
       if (packed) return launch_march_shape<f32x2, D, RS, STAGE, NWXV, 1, 1>(Uin, Ubase, Uout, g, sc, stream, depth); \
     return launch_march_shape<Real, D, RS, STAGE, NWXV, 1, minb>(Uin, Ubase, Uout, g, sc, stream, depth);           \
   }
+      if (tma && nwx == 4) return launch_march_shape<Real, D, RS, STAGE, 4, 1, minb, true>(Uin, Ubase, Uout, g, sc, stream, depth);
       PH_SHAPE(2) PH_SHAPE(3) PH_SHAPE(4) PH_SHAPE(7) PH_SHAPE(8)
 #undef PH_SHAPE
       return false;
@@ -599,6 +691,7 @@ bool launch_march_stage(const Real* Uin, const Real* Ubase, Real* Uout, const Ge
       if (packed) return launch_march_shape<f32x2, D, RS, STAGE, 1, TYV, 1>(Uin, Ubase, Uout, g, sc, stream, depth);  \
     return launch_march_shape<Real, D, RS, STAGE, 1, TYV, (TYV > 8 ? 1 : minb)>(Uin, Ubase, Uout, g, sc, stream, depth);            \
   }
+      if (tma && ty == 7) return launch_march_shape<Real, D, RS, STAGE, 1, 7, minb, true>(Uin, Ubase, Uout, g, sc, stream, depth);
       PH_SHAPE(4) PH_SHAPE(7) PH_SHAPE(8) PH_SHAPE(15)
 #undef PH_SHAPE
       return false;

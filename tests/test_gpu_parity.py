@@ -318,3 +318,17 @@ def test_heun_integrator_option_matches_oracle(gpu, oracle_mod, variant, dims, d
     assert abs(tg - t) <= 20 * TOL[np.dtype(dtype)][2] * t
     assert np.all(field_errors(got, ref) <= 11 * tol1), field_errors(got, ref)
     assert np.array_equal(got, ref)
+
+
+@pytest.mark.parametrize("boundary", ["periodic", "outflow"])
+@pytest.mark.parametrize("dims,shape", [(2, (256, 45)), (2, (300, 33)), (3, (64, 30, 21)), (3, (96, 13, 150)), (3, (40, 9, 9))])
+def test_march_tma_staging_matches_oracle(gpu, oracle_mod, dims, shape, boundary):
+    """staging = 2: the tile rows of U_in / U_base arrive by TMA bulk copies in a shared-memory ring (tiles that end
+    inside the grid; ragged tiles and n_x not a multiple of 16 bytes take the per-thread loads)."""
+    for dtype in (np.float32, np.float64):
+        w = inputs.random_smooth(shape, dtype, seed=41 + dims, boundary=boundary)
+        ref, rdt = oracle_steps(oracle_mod, w, 3)
+        for depth in (0, 5):
+            got, gdt = gpu_steps(gpu, w, 3, "march", staging=2, tile_depth=depth)
+            assert np.array_equal(got, ref), (shape, dtype, depth, field_errors(got, ref))
+            assert all(abs(a - b) <= TOL[np.dtype(dtype)][2] * b for a, b in zip(gdt, rdt))
