@@ -280,8 +280,8 @@ def roofline_of(w, r, peak, peak_src, traffic=None):
 
 
 def ncu_traffic(cfg, variant):
-    if cfg in (1, 2) and variant == "fused":
-        variant = "fused1"  # 2-D grids: the default on-chip variant is k_fused
+    if cfg == 2 and variant == "fused":
+        variant = "fused1"  # 2-D fp64 grids: the default on-chip variant is k_fused
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, copied by hand from the
     committed ncu --set full summary (profiles/traffic.csv names it); None if that variant was not captured."""
     p = os.path.join(ROOT, "profiles", "traffic.csv")

@@ -62,8 +62,8 @@ int paraiso_hydro_destroy(paraiso_hydro_t *h);
  *   "boundary"  0 periodic: index wrap (default) | 1 outflow: zero-gradient, index clamp   (R12)
  *   "riemann"   0 HLLC (default; Eq. 22) | 1 HLL                              (R4)
  *   "variant"   kernel arrangement on the paper's Manifest <-> Delayed axis (Table 5):
- *               0 fused       one kernel per RK stage, intermediates on chip (default): k_march on 3-D grids,
- *                             k_fused on 2-D grids, k_delayed in 1-D
+ *               0 fused       one kernel per RK stage, intermediates on chip (default): k_march on 3-D grids and on
+ *                             2-D fp32 grids, k_fused on 2-D fp64 grids, k_delayed in 1-D
  *               4 march       force k_march (halo warp + warp-shuffle exchange; "cells_per_thread" 2 = packed f32x2)
  *               5 fused1      force k_fused (the first on-chip design)
  *               1 manifest_flux  fluxes F_a materialised in HBM, then an update kernel

@@ -316,11 +316,14 @@ static bool launch_fused_shape(const Real* Uin, const Real* Ubase, Real* Uout, c
                                cudaStream_t stream, int depth) {
   using Smem = FusedSmem<Real, D, TX, TY>;
   auto kern = k_fused<Real, D, RS, STAGE, TX, TY>;
-  static bool configured = false;
-  if (!configured) {
+  // the opt-in to more than 48 KB of dynamic shared memory is a per-device attribute of the kernel
+  static bool configured[64] = {};
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return false;
+  if (!configured[dev]) {
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem)) != cudaSuccess)
       return false;
-    configured = true;
+    configured[dev] = true;
   }
   constexpr int M = D - 1;
   dim3 grid, block(TX, TY, 1);

@@ -619,11 +619,14 @@ static bool launch_march_shape(const scalar_t<T>* Uin, const scalar_t<T>* Ubase,
                                const Geom<scalar_t<T>>& g, Scalars* sc, cudaStream_t stream, int depth) {
   using Sh = MarchShape<T, D, NWX, TY, TMA>;
   auto kern = k_march<T, D, RS, STAGE, NWX, TY, MINB, TMA>;
-  static bool configured = false;
-  if (!configured) {
+  // the opt-in to more than 48 KB of dynamic shared memory is a per-device attribute of the kernel
+  static bool configured[64] = {};
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return false;
+  if (!configured[dev]) {
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(typename Sh::Smem)) != cudaSuccess)
       return false;
-    configured = true;
+    configured[dev] = true;
   }
   constexpr int M = D - 1;
   dim3 grid, block(Sh::NT, 1, 1);

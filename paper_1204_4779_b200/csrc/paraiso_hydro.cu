@@ -248,9 +248,10 @@ struct Launch {
         update<STAGE>(h, g, Uout);
         break;
       }
-      case VARIANT_FUSED:  // the faster of the two on-chip designs per grid kind: 3-D k_march, 2-D k_fused
+      case VARIANT_FUSED:  // the faster of the two on-chip designs per grid kind (profiles/r1d_tune_*.txt):
+                           // k_march in 3-D and in 2-D fp32, k_fused in 2-D fp64
       case VARIANT_MARCH:
-        if ((h->variant == VARIANT_MARCH || D == 3) &&
+        if ((h->variant == VARIANT_MARCH || D == 3 || sizeof(Real) == 4) &&
             launch_march_stage<Real, D, RS, STAGE>(Uin, stage_base<STAGE>(h), Uout, g, h->sc, h->stream, h->block,
                                                    h->tile_depth, h->cells_per_thread, h->staging)) {
           h->launches += 1;
