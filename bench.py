@@ -11,9 +11,11 @@ are added to the same JSON line under "all_configs" (short runs; config 1 is L2-
   value     cells * steps / device time (CUDA events on the handle's stream, max over ranks), state resident in HBM
   e2e       same metric through the C ABI with HOST (pinned) buffers: set_state(host) + cfl_dt + step +
             get_state(host) every step, copies inside the timed region
-  roofline  dominant kernel = the RK stage kernel; algorithmic bytes per launch = 2*nf*w*N (state read once,
-            written once per stage; north_star's definition) / average stage duration measured
-            with CUDA events around every stage launch inside the timed region; peak = MEASURED_PEAKS.json
+  roofline  dominant kernel = the RK stage kernel, duration = CUDA events around every stage launch inside the timed
+            region.  north_star's roofline is the slower of (a) 2*nf*w*N algorithmic bytes per launch over the measured
+            copy bandwidth (MEASURED_PEAKS.json) and (b) the counted arithmetic of DESIGN.md §8 over the FP32 / FP64
+            lane rate; the binding one is reported as `bound`, the other under `other_bound`; `traffic` = ncu DRAM
+            bytes per launch (profiles/traffic.csv); `issue_cost_cycles` = measured issue cost per instruction class
   cpu_baseline  the oracle as it stands, single-threaded and OpenMP, on a bounded sample of the same workload
 
 N > 1: replicas only (DESIGN.md §9): every rank advances its own copy of the workload, no data-path collective;
