@@ -69,7 +69,10 @@ int paraiso_hydro_destroy(paraiso_hydro_t *h);
  *               1 manifest_flux  fluxes F_a materialised in HBM, then an update kernel
  *               2 manifest_all   V, VL/VR and F_a all materialised in HBM, one kernel per piece
  *               3 delayed     one kernel per stage, every thread recomputes all it needs from U
- *   "block_x" "block_y" "block_z" "tile_depth" "cells_per_thread"   launch-shape knobs of the sweep (0 = default)
+ *   "block_x" "block_y" "block_z" "tile_depth" "cells_per_thread"   launch-shape knobs of the sweep (0 = default):
+ *               k_fused: block_x x block_y = tile; k_march: block_x = main warps per row (2-D), block_y = main warps
+ *               (3-D), block_z = rows per main thread (3-D: 1 or 2), cells_per_thread 2 = packed f32x2;
+ *               tile_depth = planes marched per block
  *   "graph"     1 replay steps of run() from a captured CUDA graph (default) | 0 plain launches
  *   "staging"   k_march only: 0 / 1 every thread loads its own cells (default) | 2 TMA bulk copies of the tile rows into a
  *               shared-memory ring (one cell per thread, n_x a multiple of 16 bytes; measured slower)

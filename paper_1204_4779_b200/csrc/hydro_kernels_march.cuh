@@ -79,27 +79,25 @@ __device__ __forceinline__ int bad_lanes(const Prim<T, D>& V, T E) {
   return lane_count(m_or(m_or(m_not(gt(V.rho, zero)), m_not(gt(V.p, zero))), m_not(le(rabs(E), T(S(3.0e38))))));
 }
 
-template <class T, int D, int NWX, int TY, bool TMA = false>
+template <class T, int D, int NWX, int TY, bool TMA = false, int RPT = 1>
 struct MarchShape {
   using S = scalar_t<T>;
   static constexpr int W = LaneTraits<T>::W;
   static constexpr int NF = D + 2;
   static constexpr int TXC = NWX * 32 * W;              // cells per tile row
   static constexpr int PX = TXC + 4;                    // plane row: tile + 2 halo cells on each side
-  static constexpr int PY = (D == 3) ? TY + 4 : 1;
+  static constexpr int TYC = TY * RPT;                  // tile rows: RPT rows per main warp
+  static constexpr int PY = (D == 3) ? TYC + 4 : 1;
   static constexpr int OY = (D == 3) ? 2 : 0;           // plane row of the tile's first row
   static constexpr int NMAIN = NWX * TY * 32;           // main threads; the halo warp follows them
   static constexpr int NT = NMAIN + 32;
-  static constexpr int XROWS = (D == 3) ? TY : 1;       // tile rows = x halo tasks per plane
+  static constexpr int XROWS = (D == 3) ? TYC : 1;      // tile rows = x halo tasks per plane
   static constexpr int XTASK_LANES = (XROWS + W - 1) / W;
   static constexpr int XHALO_LANES = 4 * XROWS / W;     // lanes of the halo warp that load x halo cells
   static_assert(D == 2 || D == 3, "the marching kernel covers 2-D and 3-D grids");
   static_assert(D == 3 || TY == 1, "2-D tiles are rows");
   static_assert(D == 2 || NWX == 1, "3-D tiles are one warp wide");
-  // who fills the four y halo rows of the plane: four of the main warps, or the halo warp (which then carries
-  // about as many instructions per plane as a main warp: the four schedulers of the SM stay evenly loaded)
-  static constexpr bool YH_MAIN = false;
-  static_assert(D == 2 || !YH_MAIN || TY >= 4, "four different main warps fill the y halo rows");
+  static_assert(RPT == 1 || (D == 3 && RPT == 2 && !TMA), "two rows per thread: 3-D, per-thread loads");
   static_assert(XTASK_LANES <= 32, "tile too tall for one halo warp");
   static constexpr int RING = 4;                        // TMA: raw planes m .. m+3 of the tile's own cells
   struct Smem {
@@ -110,8 +108,8 @@ struct MarchShape {
     S Ub[TMA ? 2 : 1][TMA ? NF : 1][TMA ? XROWS : 1][TMA ? TXC : 4];
     unsigned long long mbar[RING + 2];
     S V[2][NF][PY][PX];                                 // primitives of plane m (double-buffered), halo 2
-    S LOy[(D == 3) ? NF : 1][TY + 1][(D == 3) ? TXC : 2];  // [r]: low-side y state of tile row r (r = TY: halo warp)
-    S Fy[(D == 3) ? NF : 1][TY][(D == 3) ? TXC : 2];    // [r]: flux through the low y face of tile row r (r = 0: halo warp)
+    S LOy[(D == 3) ? NF : 1][TYC + 1][(D == 3) ? TXC : 2];  // [r]: low-side y state of tile row r (r = TYC: halo warp)
+    S Fy[(D == 3) ? NF : 1][TYC][(D == 3) ? TXC : 2];   // [r]: flux through the low y face of tile row r (r = 0: halo warp)
     S LOx[NF][XROWS][NWX + 1];                          // [e]: low-side x state of the first cell of warp column e (e = NWX: halo warp)
     S Fx[NF][XROWS][NWX];                               // [e]: flux through the low x face of warp column e (e = 0: halo warp)
   };
@@ -207,14 +205,14 @@ __device__ __forceinline__ void block_barrier() { __syncwarp(); }
 __device__ __forceinline__ void block_barrier() { asm volatile("bar.sync 0;" ::: "memory"); }
 #endif
 
-template <class T, int D, int RS, int STAGE, int NWX, int TY, int MINB, bool TMA>
-__global__ void __launch_bounds__(MarchShape<T, D, NWX, TY, TMA>::NT, MINB)
+template <class T, int D, int RS, int STAGE, int NWX, int TY, int MINB, bool TMA, int RPT>
+__global__ void __launch_bounds__(MarchShape<T, D, NWX, TY, TMA, RPT>::NT, MINB)
     k_march(const scalar_t<T>* __restrict__ Uin, const scalar_t<T>* Ubase, scalar_t<T>* Uout, Geom<scalar_t<T>> g,
             Scalars* sc, int depth) {
-  using Sh = MarchShape<T, D, NWX, TY, TMA>;
+  using Sh = MarchShape<T, D, NWX, TY, TMA, RPT>;
   using S = scalar_t<T>;
   using P = Prim<T, D>;
-  constexpr int W = Sh::W, NF = Sh::NF, TXC = Sh::TXC, OY = Sh::OY, XROWS = Sh::XROWS;
+  constexpr int W = Sh::W, NF = Sh::NF, TXC = Sh::TXC, OY = Sh::OY, XROWS = Sh::XROWS, TYC = Sh::TYC;
   constexpr int M = D - 1;  // marching axis
   constexpr int RING = Sh::RING;
 
@@ -225,7 +223,7 @@ __global__ void __launch_bounds__(MarchShape<T, D, NWX, TY, TMA>::NT, MINB)
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int nx = g.n[0], ny = g.n[1], nM = g.n[M], bnd = g.boundary;
   const int x0 = blockIdx.x * TXC;
-  const int y0 = (D == 3) ? blockIdx.y * TY : 0;
+  const int y0 = (D == 3) ? blockIdx.y * TYC : 0;
   const int bm = (D == 3) ? blockIdx.z : blockIdx.y;
   const int m0 = bm * depth;
   const int m1 = min(m0 + depth, nM);
@@ -242,18 +240,24 @@ __global__ void __launch_bounds__(MarchShape<T, D, NWX, TY, TMA>::NT, MINB)
 
   if (warp < NWX * TY) {
     // =========================================================================== main warps
-    const int row = (D == 3) ? warp : 0;
+    // A thread owns RPT cells of one x position: tile rows RPT*warp .. RPT*warp + RPT-1 (3-D; RPT = 1 in 2-D).  With
+    // RPT = 2 the y face between its two cells never leaves the registers and the halo warp serves twice the rows.
     const int wx = (D == 3) ? 0 : warp;
     const int c0 = (wx * 32 + lane) * W;  // first own cell, tile coordinates
-    const int gi = x0 + c0, gj = y0 + row;
-    const bool active = gi < nx && (D == 2 || gj < ny);
-    const CellSrc src = cell_src<T>(gi, grid_row(gj), nx, bnd);
-    const int own = (D == 3 ? gj * nx : 0) + gi;  // valid when active
-    const int pr = row + OY, pc = c0 + 2;         // own position in the shared plane
-    // 3-D: the first two and the last two main warps also fill one y halo row of the plane each
-    const int yh_py = (D == 3 && Sh::YH_MAIN) ? (row == 0 ? 0 : row == 1 ? 1 : row == TY - 2 ? TY + 2 : row == TY - 1 ? TY + 3 : -1) : -1;
-    const bool yh = yh_py >= 0;
-    const CellSrc yh_src = cell_src<T>(gi, grid_row(y0 + (yh ? yh_py : 2) - 2), nx, bnd);
+    const int gi = x0 + c0;
+    const int pc = c0 + 2;                // own column in the shared plane
+    int row[RPT], pr[RPT], own[RPT];
+    bool active[RPT];
+    CellSrc src[RPT];
+#pragma unroll
+    for (int rr = 0; rr < RPT; ++rr) {
+      row[rr] = (D == 3) ? warp * RPT + rr : 0;
+      const int gj = y0 + row[rr];
+      active[rr] = gi < nx && (D == 2 || gj < ny);
+      src[rr] = cell_src<T>(gi, grid_row(gj), nx, bnd);
+      own[rr] = (D == 3 ? gj * nx : 0) + gi;  // valid when active
+      pr[rr] = row[rr] + OY;
+    }
 
     auto load_cells_of = [&](const CellSrc& c, int m, T (&u)[NF]) {
       const int pl = plane_of(m);
@@ -266,177 +270,192 @@ __global__ void __launch_bounds__(MarchShape<T, D, NWX, TY, TMA>::NT, MINB)
 #pragma unroll
       for (int f = 0; f < NF; ++f) sts(&sm.V[b][f][py][pc], u[f]);
     };
+    auto lds_plane = [&](int b, int py) {
+      T u[NF];
+#pragma unroll
+      for (int f = 0; f < NF; ++f) u[f] = lds<T>(&sm.V[b][f][py][pc]);
+      return prim_from_fields<T, D>(u);
+    };
 
     const S lam0 = S(sc->lam[STAGE - 1][0]);
     const S lam1 = S(sc->lam[STAGE - 1][1]);
     const S lam2 = (D == 3) ? S(sc->lam[STAGE - 1][2]) : S(0);
 
     // ---- prologue: rolling window at m0
-    P Vc, Vp1, hiM;
-    T Fprev[NF], Unext[NF];
-    {
+    P Vc[RPT], Vp1[RPT], hiM[RPT];
+    T Fprev[RPT][NF], Unext[RPT][NF];
+#pragma unroll
+    for (int rr = 0; rr < RPT; ++rr) {
       T u[NF];
-      load_cells_of(src, m0 - 2, u);
+      load_cells_of(src[rr], m0 - 2, u);
       const P Vm2 = prim_of<T, D>(u, g.gm1);
-      load_cells_of(src, m0 - 1, u);
+      load_cells_of(src[rr], m0 - 1, u);
       const P Vm1 = prim_of<T, D>(u, g.gm1);
-      load_cells_of(src, m0, u);
-      Vc = prim_of<T, D>(u, g.gm1);
-      load_cells_of(src, m0 + 1, u);
-      Vp1 = prim_of<T, D>(u, g.gm1);
-      if (!use_tma) load_cells_of(src, m0 + 2, Unext);
+      load_cells_of(src[rr], m0, u);
+      Vc[rr] = prim_of<T, D>(u, g.gm1);
+      load_cells_of(src[rr], m0 + 1, u);
+      Vp1[rr] = prim_of<T, D>(u, g.gm1);
+      if (!use_tma) load_cells_of(src[rr], m0 + 2, Unext[rr]);
       P him1, loc;
-      interpolate<T, D>(Vm2, Vm1, Vc, nullptr, &him1);
-      interpolate<T, D>(Vm1, Vc, Vp1, &loc, &hiM);
-      riemann_flux<T, D, M, RS>(g.gamma, g.igm1, him1, loc, Fprev);
-      sts_plane(0, pr, Vc);
-      if (yh) {
-        load_cells_of(yh_src, m0, u);
-        sts_plane(0, yh_py, prim_of<T, D>(u, g.gm1));
-      }
+      interpolate<T, D>(Vm2, Vm1, Vc[rr], nullptr, &him1);
+      interpolate<T, D>(Vm1, Vc[rr], Vp1[rr], &loc, &hiM[rr]);
+      riemann_flux<T, D, M, RS>(g.gamma, g.igm1, him1, loc, Fprev[rr]);
+      sts_plane(0, pr[rr], Vc[rr]);
     }
     block_barrier();
 
     int b = 0;
     for (int m = m0; m < m1; ++m, b ^= 1) {
       const bool more = m + 1 < m1;
+      const int q = m - m0;  // plane index inside this block's march
       // ------------------------------------------------------------ phase A: slopes, the marching-axis face
-      P hix, lox, hiy;
-      {
+      P hix[RPT], lox[RPT], hiy[RPT], loy_up;  // loy_up (RPT = 2): low-side y state of the thread's upper cell
+#pragma unroll
+      for (int rr = 0; rr < RPT; ++rr) {
         T vc[NF], l[NF], r[NF];
-        prim_to_fields<T, D>(Vc, vc);
+        prim_to_fields<T, D>(Vc[rr], vc);
 #pragma unroll
         for (int f = 0; f < NF; ++f) {
-          l[f] = xshift_left(vc[f], sm.V[b][f][pr][pc - 1]);
-          r[f] = xshift_right(vc[f], sm.V[b][f][pr][pc + W]);
+          l[f] = xshift_left(vc[f], sm.V[b][f][pr[rr]][pc - 1]);
+          r[f] = xshift_right(vc[f], sm.V[b][f][pr[rr]][pc + W]);
         }
-        interpolate<T, D>(prim_from_fields<T, D>(l), Vc, prim_from_fields<T, D>(r), &lox, &hix);
+        interpolate<T, D>(prim_from_fields<T, D>(l), Vc[rr], prim_from_fields<T, D>(r), &lox[rr], &hix[rr]);
         if (lane == 0) {  // low-side state of this warp column's first cell, for the warp (or halo task) on its left
           T a[NF];
-          prim_to_fields<T, D>(lox, a);
+          prim_to_fields<T, D>(lox[rr], a);
 #pragma unroll
-          for (int f = 0; f < NF; ++f) sm.LOx[f][row][wx] = lane_first(a[f]);
+          for (int f = 0; f < NF; ++f) sm.LOx[f][row[rr]][wx] = lane_first(a[f]);
         }
       }
       if constexpr (D == 3) {
-        T d[NF], u[NF];
-#pragma unroll
-        for (int f = 0; f < NF; ++f) {
-          d[f] = lds<T>(&sm.V[b][f][pr - 1][pc]);
-          u[f] = lds<T>(&sm.V[b][f][pr + 1][pc]);
-        }
+        // y slopes: neighbours inside the thread come from registers, the others from the shared plane
         P loy;
-        interpolate<T, D>(prim_from_fields<T, D>(d), Vc, prim_from_fields<T, D>(u), &loy, &hiy);
+        if constexpr (RPT == 1) {
+          interpolate<T, D>(lds_plane(b, pr[0] - 1), Vc[0], lds_plane(b, pr[0] + 1), &loy, &hiy[0]);
+        } else {
+          interpolate<T, D>(lds_plane(b, pr[0] - 1), Vc[0], Vc[1], &loy, &hiy[0]);
+          interpolate<T, D>(Vc[0], Vc[1], lds_plane(b, pr[1] + 1), &loy_up, &hiy[1]);
+        }
         T a[NF];
         prim_to_fields<T, D>(loy, a);
 #pragma unroll
-        for (int f = 0; f < NF; ++f) sts(&sm.LOy[f][row][c0], a[f]);
+        for (int f = 0; f < NF; ++f) sts(&sm.LOy[f][row[0]][c0], a[f]);
       }
       // marching axis: V[m+2], slope of cell m+1, flux through face m+1/2
-      const int q = m - m0;  // plane index inside this block's march
-      if (TMA && use_tma) {  // U_in of plane m+2: landed in ring slot (q+2) % RING one iteration ago
-        mbar_wait(&sm.mbar[(q + 2) % RING], ((q + 2) / RING) & 1);
+      P Vp2[RPT], hiM1[RPT];
+      T Fnext[RPT][NF];
 #pragma unroll
-        for (int f = 0; f < NF; ++f) Unext[f] = lds<T>(&sm.Uraw[(q + 2) % RING][f][row][c0]);
+      for (int rr = 0; rr < RPT; ++rr) {
+        if (TMA && use_tma) {  // U_in of plane m+2: landed in ring slot (q+2) % RING one iteration ago
+          mbar_wait(&sm.mbar[(q + 2) % RING], ((q + 2) / RING) & 1);
+#pragma unroll
+          for (int f = 0; f < NF; ++f) Unext[rr][f] = lds<T>(&sm.Uraw[(q + 2) % RING][f][row[rr]][c0]);
+        }
+        Vp2[rr] = prim_of<T, D>(Unext[rr], g.gm1);
+        if (more && !use_tma) load_cells_of(src[rr], m + 3, Unext[rr]);
+        P loM1;
+        interpolate<T, D>(Vc[rr], Vp1[rr], Vp2[rr], &loM1, &hiM1[rr]);
+        riemann_flux<T, D, M, RS>(g.gamma, g.igm1, hiM[rr], loM1, Fnext[rr]);
+        if (more) sts_plane(b ^ 1, pr[rr], Vp1[rr]);
       }
-      const P Vp2 = prim_of<T, D>(Unext, g.gm1);
-      if (more && !use_tma) load_cells_of(src, m + 3, Unext);
-      P loM1, hiM1;
-      interpolate<T, D>(Vc, Vp1, Vp2, &loM1, &hiM1);
-      T Fnext[NF];
-      riemann_flux<T, D, M, RS>(g.gamma, g.igm1, hiM, loM1, Fnext);
-      if (more) sts_plane(b ^ 1, pr, Vp1);
       block_barrier();
 
       // ------------------------------------------------------------ phase B: one Riemann solve per in-plane face
-      T Uy[NF];
-      if (yh && more) load_cells_of(yh_src, m + 1, Uy);
-      T Fx[NF], Fy[NF];
-      {
+      T Fx[RPT][NF], Fy[RPT][NF];  // Fy[rr]: flux through the upper y face of the thread's cell rr
+#pragma unroll
+      for (int rr = 0; rr < RPT; ++rr) {
         T a[NF], rs[NF];
-        prim_to_fields<T, D>(lox, a);
+        prim_to_fields<T, D>(lox[rr], a);
 #pragma unroll
         for (int f = 0; f < NF; ++f) {
           S nb = shfl_dn(lane_first(a[f]));
-          if (lane == 31) nb = sm.LOx[f][row][wx + 1];
+          if (lane == 31) nb = sm.LOx[f][row[rr]][wx + 1];
           rs[f] = xshift_right(a[f], nb);
         }
-        riemann_flux<T, D, 0, RS>(g.gamma, g.igm1, hix, prim_from_fields<T, D>(rs), Fx);
+        riemann_flux<T, D, 0, RS>(g.gamma, g.igm1, hix[rr], prim_from_fields<T, D>(rs), Fx[rr]);
         if (NWX > 1 && lane == 31 && wx + 1 < NWX) {
 #pragma unroll
-          for (int f = 0; f < NF; ++f) sm.Fx[f][row][wx + 1] = lane_last(Fx[f]);
+          for (int f = 0; f < NF; ++f) sm.Fx[f][row[rr]][wx + 1] = lane_last(Fx[rr][f]);
         }
       }
       if constexpr (D == 3) {
+        if constexpr (RPT == 2) riemann_flux<T, D, 1, RS>(g.gamma, g.igm1, hiy[0], loy_up, Fy[0]);
         T a[NF];
 #pragma unroll
-        for (int f = 0; f < NF; ++f) a[f] = lds<T>(&sm.LOy[f][row + 1][c0]);
-        riemann_flux<T, D, 1, RS>(g.gamma, g.igm1, hiy, prim_from_fields<T, D>(a), Fy);
-        if (row + 1 < TY) {
+        for (int f = 0; f < NF; ++f) a[f] = lds<T>(&sm.LOy[f][row[RPT - 1] + 1][c0]);
+        riemann_flux<T, D, 1, RS>(g.gamma, g.igm1, hiy[RPT - 1], prim_from_fields<T, D>(a), Fy[RPT - 1]);
+        if (row[RPT - 1] + 1 < TYC) {
 #pragma unroll
-          for (int f = 0; f < NF; ++f) sts(&sm.Fy[f][row + 1][c0], Fy[f]);
+          for (int f = 0; f < NF; ++f) sts(&sm.Fy[f][row[RPT - 1] + 1][c0], Fy[RPT - 1][f]);
         }
       }
       // own-cell base state of Eq. 23 (coherent load: the last stage overwrites U_base in place)
-      const int cell = plane_of(m) + own;
-      T u[NF];
-      if (TMA && use_tma) {  // stage 1: U_base = U_in, plane m of the ring; last stage: the U0 ring
-        if (STAGE == 1) {
-          mbar_wait(&sm.mbar[q % RING], (q / RING) & 1);
+      const int pl = plane_of(m);
+      T u[RPT][NF];
 #pragma unroll
-          for (int f = 0; f < NF; ++f) u[f] = lds<T>(&sm.Uraw[q % RING][f][row][c0]);
-        } else {
-          mbar_wait(&sm.mbar[RING + (q & 1)], (q >> 1) & 1);
+      for (int rr = 0; rr < RPT; ++rr) {
+        if (TMA && use_tma) {  // stage 1: U_base = U_in, plane m of the ring; last stage: the U0 ring
+          if (STAGE == 1) {
+            mbar_wait(&sm.mbar[q % RING], (q / RING) & 1);
 #pragma unroll
-          for (int f = 0; f < NF; ++f) u[f] = lds<T>(&sm.Ub[q & 1][f][row][c0]);
+            for (int f = 0; f < NF; ++f) u[rr][f] = lds<T>(&sm.Uraw[q % RING][f][row[rr]][c0]);
+          } else {
+            mbar_wait(&sm.mbar[RING + (q & 1)], (q >> 1) & 1);
+#pragma unroll
+            for (int f = 0; f < NF; ++f) u[rr][f] = lds<T>(&sm.Ub[q & 1][f][row[rr]][c0]);
+          }
+        } else if (active[rr]) {
+#pragma unroll
+          for (int f = 0; f < NF; ++f) u[rr][f] = ld_cells_rw<T>(Ubase, f * Ni + pl + own[rr]);
         }
-      } else if (active) {
-#pragma unroll
-        for (int f = 0; f < NF; ++f) u[f] = ld_cells_rw<T>(Ubase, f * Ni + cell);
       }
-      if (yh && more) sts_plane(b ^ 1, yh_py, prim_of<T, D>(Uy, g.gm1));
       block_barrier();
 
       // ------------------------------------------------------------ phase C: Eq. 23, axes in the order x, y, z
-      {
+#pragma unroll
+      for (int rr = 0; rr < RPT; ++rr) {
         T lowx[NF];
 #pragma unroll
         for (int f = 0; f < NF; ++f) {
-          S nb = shfl_up(lane_last(Fx[f]));
-          if (lane == 0) nb = sm.Fx[f][row][wx];
-          lowx[f] = xshift_left(Fx[f], nb);
+          S nb = shfl_up(lane_last(Fx[rr][f]));
+          if (lane == 0) nb = sm.Fx[f][row[rr]][wx];
+          lowx[f] = xshift_left(Fx[rr][f], nb);
         }
-        if (active) {
+        if (active[rr]) {
+          const int cell = pl + own[rr];
 #pragma unroll
-          for (int f = 0; f < NF; ++f) u[f] = rfma(lam0, lowx[f] - Fx[f], u[f]);
+          for (int f = 0; f < NF; ++f) u[rr][f] = rfma(lam0, lowx[f] - Fx[rr][f], u[rr][f]);
           if constexpr (D == 3) {
 #pragma unroll
-            for (int f = 0; f < NF; ++f) u[f] = rfma(lam1, lds<T>(&sm.Fy[f][row][c0]) - Fy[f], u[f]);
+            for (int f = 0; f < NF; ++f) {
+              const T lowy = (rr == 0) ? lds<T>(&sm.Fy[f][row[0]][c0]) : Fy[0][f];
+              u[rr][f] = rfma(lam1, lowy - Fy[rr][f], u[rr][f]);
+            }
 #pragma unroll
-            for (int f = 0; f < NF; ++f) u[f] = rfma(lam2, Fprev[f] - Fnext[f], u[f]);
+            for (int f = 0; f < NF; ++f) u[rr][f] = rfma(lam2, Fprev[rr][f] - Fnext[rr][f], u[rr][f]);
           } else {
 #pragma unroll
-            for (int f = 0; f < NF; ++f) u[f] = rfma(lam1, Fprev[f] - Fnext[f], u[f]);
+            for (int f = 0; f < NF; ++f) u[rr][f] = rfma(lam1, Fprev[rr][f] - Fnext[rr][f], u[rr][f]);
           }
           if (STAGE == 2 && g.integrator == 1) {  // Heun: U2 = 0.5 (U0 + (U1 + dt L(U1))); U0 still sits in Uout
 #pragma unroll
-            for (int f = 0; f < NF; ++f) u[f] = S(0.5) * (ld_cells_rw<T>(Uout, f * Ni + cell) + u[f]);
+            for (int f = 0; f < NF; ++f) u[rr][f] = S(0.5) * (ld_cells_rw<T>(Uout, f * Ni + cell) + u[rr][f]);
           }
 #pragma unroll
-          for (int f = 0; f < NF; ++f) st_cells<T>(Uout, f * Ni + cell, u[f]);
+          for (int f = 0; f < NF; ++f) st_cells<T>(Uout, f * Ni + cell, u[rr][f]);
           if (STAGE == 2) {
             T ir;
-            const P Vn = prim_of<T, D>(u, g.gm1, &ir);
+            const P Vn = prim_of<T, D>(u[rr], g.gm1, &ir);
             s_max = rmax(s_max, lane_max(cfl_speed<T, D>(Vn, ir, g.gamma, g.idr)));
-            bad += bad_lanes<T, D>(Vn, u[NF - 1]);
+            bad += bad_lanes<T, D>(Vn, u[rr][NF - 1]);
           }
         }
-      }
 #pragma unroll
-      for (int f = 0; f < NF; ++f) Fprev[f] = Fnext[f];
-      Vc = Vp1;
-      Vp1 = Vp2;
-      hiM = hiM1;
+        for (int f = 0; f < NF; ++f) Fprev[rr][f] = Fnext[rr][f];
+        Vc[rr] = Vp1[rr];
+        Vp1[rr] = Vp2[rr];
+        hiM[rr] = hiM1[rr];
+      }
     }
   } else {
     // =========================================================================== the halo warp
@@ -464,10 +483,10 @@ __global__ void __launch_bounds__(MarchShape<T, D, NWX, TY, TMA>::NT, MINB)
       hpx[q] = px;
       hsrc[q] = cell_src<T>(x0 + px - 2, grid_row(y0 + r), nx, bnd);
     }
-    constexpr int NYP = (D == 3 && !Sh::YH_MAIN) ? 4 : 0;  // y halo rows this warp fills
+    constexpr int NYP = (D == 3) ? 4 : 0;  // y halo rows this warp fills
     CellSrc ysrc[NYP > 0 ? NYP : 1];
 #pragma unroll
-    for (int q = 0; q < NYP; ++q) ysrc[q] = cell_src<T>(x0 + lane * W, grid_row(y0 + (q < 2 ? q : TY + q) - 2), nx, bnd);
+    for (int q = 0; q < NYP; ++q) ysrc[q] = cell_src<T>(x0 + lane * W, grid_row(y0 + (q < 2 ? q : TYC + q) - 2), nx, bnd);
     T Uh[NXP][NF], Uyh[NYP > 0 ? NYP : 1][NF];
     auto load_halo = [&](int m) {
       const int pl = plane_of(m);
@@ -496,7 +515,7 @@ __global__ void __launch_bounds__(MarchShape<T, D, NWX, TY, TMA>::NT, MINB)
       for (int q = 0; q < NYP; ++q) {
         prim_to_fields<T, D>(prim_of<T, D>(Uyh[q], g.gm1), u);
 #pragma unroll
-        for (int f = 0; f < NF; ++f) sts(&sm.V[b][f][q < 2 ? q : TY + q][lane * W + 2], u[f]);
+        for (int f = 0; f < NF; ++f) sts(&sm.V[b][f][q < 2 ? q : TYC + q][lane * W + 2], u[f]);
       }
     };
     // x face tasks: lane l < XTASK_LANES handles tile rows ra (first lane of T) and rb (second lane)
@@ -563,11 +582,11 @@ __global__ void __launch_bounds__(MarchShape<T, D, NWX, TY, TMA>::NT, MINB)
       if constexpr (D == 3) {
         interpolate<T, D>(plane_y(b, 0), plane_y(b, 1), plane_y(b, 2), nullptr, &hiYlow);
         P lo;
-        interpolate<T, D>(plane_y(b, TY + 1), plane_y(b, TY + 2), plane_y(b, TY + 3), &lo, nullptr);
+        interpolate<T, D>(plane_y(b, TYC + 1), plane_y(b, TYC + 2), plane_y(b, TYC + 3), &lo, nullptr);
         T a[NF];
         prim_to_fields<T, D>(lo, a);
 #pragma unroll
-        for (int f = 0; f < NF; ++f) sts(&sm.LOy[f][TY][lane * W], a[f]);
+        for (int f = 0; f < NF; ++f) sts(&sm.LOy[f][TYC][lane * W], a[f]);
       }
       if (xtask) {
         interpolate<T, D>(plane_x(b, 0), plane_x(b, 1), plane_x(b, 2), nullptr, &hiXlow);
@@ -614,11 +633,11 @@ __global__ void __launch_bounds__(MarchShape<T, D, NWX, TY, TMA>::NT, MINB)
 }
 
 // ------------------------------------------------------------------------------------------------
-template <class T, int D, int RS, int STAGE, int NWX, int TY, int MINB, bool TMA = false>
+template <class T, int D, int RS, int STAGE, int NWX, int TY, int MINB, bool TMA = false, int RPT = 1>
 static bool launch_march_shape(const scalar_t<T>* Uin, const scalar_t<T>* Ubase, scalar_t<T>* Uout,
                                const Geom<scalar_t<T>>& g, Scalars* sc, cudaStream_t stream, int depth) {
-  using Sh = MarchShape<T, D, NWX, TY, TMA>;
-  auto kern = k_march<T, D, RS, STAGE, NWX, TY, MINB, TMA>;
+  using Sh = MarchShape<T, D, NWX, TY, TMA, RPT>;
+  auto kern = k_march<T, D, RS, STAGE, NWX, TY, MINB, TMA, RPT>;
   // the opt-in to more than 48 KB of dynamic shared memory is a per-device attribute of the kernel
   static bool configured[64] = {};
   int dev = 0;
@@ -632,7 +651,7 @@ static bool launch_march_shape(const scalar_t<T>* Uin, const scalar_t<T>* Ubase,
   dim3 grid, block(Sh::NT, 1, 1);
   grid.x = (g.n[0] + Sh::TXC - 1) / Sh::TXC;
   if (D == 3) {
-    grid.y = (g.n[1] + TY - 1) / TY;
+    grid.y = (g.n[1] + Sh::TYC - 1) / Sh::TYC;
     grid.z = (g.n[M] + depth - 1) / depth;
     if (grid.y > 65535u || grid.z > 65535u) return false;
   } else {
@@ -655,7 +674,8 @@ inline int march_default_depth(long long tiles_in_plane, int nM) {
 // Returns false when the marching kernel does not cover this shape (the caller falls back).
 //   pack: cells per thread along x (0 = default = 1; 2 = packed f32x2, fp32 on an even n_x only: measured slower,
 //         DESIGN.md §7)
-//   block[0] (2-D): main warps per block (0 = default); block[1] (3-D): tile rows TY (0 = default)
+//   block[0] (2-D): main warps per block (0 = default); block[1] (3-D): main warps TY (0 = default);
+//   block[2] (3-D): rows per thread (0 / 1, or 2 with TY = 7)
 //   staging: 0 / 1 = every thread loads its own cells (LDG), 2 = TMA bulk copies of the tile rows into a shared-memory
 //            ring (one cell per thread, n_x a multiple of 16 bytes, default tile shapes only)
 template <class Real, int D, int RS, int STAGE>
@@ -695,6 +715,8 @@ bool launch_march_stage(const Real* Uin, const Real* Ubase, Real* Uout, const Ge
     return launch_march_shape<Real, D, RS, STAGE, 1, TYV, (TYV > 8 ? 1 : minb)>(Uin, Ubase, Uout, g, sc, stream, depth);            \
   }
       if (tma && ty == 7) return launch_march_shape<Real, D, RS, STAGE, 1, 7, minb, true>(Uin, Ubase, Uout, g, sc, stream, depth);
+      if (block[2] == 2 && ty == 7 && !packed)  // two rows per thread: a 32 x 14 tile, one 256-thread block per SM
+        return launch_march_shape<Real, D, RS, STAGE, 1, 7, 1, false, 2>(Uin, Ubase, Uout, g, sc, stream, depth);
       PH_SHAPE(4) PH_SHAPE(7) PH_SHAPE(8) PH_SHAPE(15)
 #undef PH_SHAPE
       return false;

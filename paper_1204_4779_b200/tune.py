@@ -32,6 +32,7 @@ def candidates(dims, dtype_is_f32):
             for ty in (7, 8):
                 out.append((f"march packed f32x2 ty={ty}", "march", {"block_y": ty, "cells_per_thread": 2}))
         out.append(("march ty=7 TMA staging", "march", {"block_y": 7, "staging": 2}))
+        out.append(("march ty=7 two rows per thread", "march", {"block_y": 7, "block_z": 2}))
     else:
         for nwx, d in itertools.product((2, 4, 8), depths):
             out.append((f"march warps={nwx} depth={d or 'auto'}", "march", {"block_x": nwx, "tile_depth": d}))

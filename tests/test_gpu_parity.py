@@ -332,3 +332,16 @@ def test_march_tma_staging_matches_oracle(gpu, oracle_mod, dims, shape, boundary
             got, gdt = gpu_steps(gpu, w, 3, "march", staging=2, tile_depth=depth)
             assert np.array_equal(got, ref), (shape, dtype, depth, field_errors(got, ref))
             assert all(abs(a - b) <= TOL[np.dtype(dtype)][2] * b for a, b in zip(gdt, rdt))
+
+
+@pytest.mark.parametrize("boundary", ["periodic", "outflow"])
+@pytest.mark.parametrize("shape", [(64, 30, 21), (45, 38, 27), (40, 13, 9), (33, 4, 5)])
+def test_march_two_rows_per_thread_matches_oracle(gpu, oracle_mod, shape, boundary):
+    """block_z = 2: a main thread owns two y-adjacent cells (32 x 14 tile); the y face between them stays in registers."""
+    for dtype in (np.float32, np.float64):
+        w = inputs.random_smooth(shape, dtype, seed=51, boundary=boundary)
+        ref, rdt = oracle_steps(oracle_mod, w, 3)
+        for depth in (0, 4):
+            got, gdt = gpu_steps(gpu, w, 3, "march", block_z=2, tile_depth=depth)
+            assert np.array_equal(got, ref), (shape, dtype, depth, field_errors(got, ref))
+            assert all(abs(a - b) <= TOL[np.dtype(dtype)][2] * b for a, b in zip(gdt, rdt))
