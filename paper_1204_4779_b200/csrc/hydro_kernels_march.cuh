@@ -23,6 +23,9 @@
 #pragma once
 #include "hydro_kernels_basic.cuh"
 
+#ifndef PH_RPT2_MINB
+#define PH_RPT2_MINB 1
+#endif
 #ifndef PH_MARCH_MINB
 #define PH_MARCH_MINB 2
 #endif
@@ -716,7 +719,7 @@ bool launch_march_stage(const Real* Uin, const Real* Ubase, Real* Uout, const Ge
   }
       if (tma && ty == 7) return launch_march_shape<Real, D, RS, STAGE, 1, 7, minb, true>(Uin, Ubase, Uout, g, sc, stream, depth);
       if (block[2] == 2 && ty == 7 && !packed)  // two rows per thread: a 32 x 14 tile, one 256-thread block per SM
-        return launch_march_shape<Real, D, RS, STAGE, 1, 7, 1, false, 2>(Uin, Ubase, Uout, g, sc, stream, depth);
+        return launch_march_shape<Real, D, RS, STAGE, 1, 7, PH_RPT2_MINB, false, 2>(Uin, Ubase, Uout, g, sc, stream, depth);
       PH_SHAPE(4) PH_SHAPE(7) PH_SHAPE(8) PH_SHAPE(15)
 #undef PH_SHAPE
       return false;
