@@ -3,10 +3,12 @@
 // sm_100a), organised around what the r1b Nsight capture of k_fused showed (profiles/r1b_README.md):
 // the stage is bound by instruction issue, not by DRAM.
 //
-//   * T = f32x2: a thread owns TWO x-adjacent cells, held in 64-bit register pairs and computed with the
-//     packed FADD2 / FMUL2 / FFMA2 instructions (one issue slot, two IEEE-rounded fp32 results, bit-identical
-//     to the scalar instructions); global and shared accesses of the pair are 64-bit; index arithmetic,
-//     loop overhead and register moves are paid once per two cells.  T = float / double: one cell per thread.
+//   * T = float / double: one cell per thread and x position (the default).  T = f32x2 (option cells_per_thread
+//     = 2): a thread owns TWO x-adjacent cells, held in 64-bit register pairs and computed with the packed
+//     FADD2 / FMUL2 / FFMA2 instructions (one issue slot, two IEEE-rounded fp32 results, bit-identical to the
+//     scalar instructions), 64-bit global and shared accesses; fewer instructions per cell but ~210 registers:
+//     measured slower, kept as an option.  Further options of the same kind: RPT = 2 (two
+//     y-adjacent cells per thread), TMA (bulk-copy staging of the tile rows into a shared-memory ring).
 //   * a block = NWX x TY "main" warps (a tile of TXC = NWX*32*W cells by TY rows of the leading plane, marched
 //     through `depth` planes of the last axis with a rolling register window, as in k_fused) + ONE halo warp.
 //     The halo warp loads the 2-cell star halo of every plane, converts it to primitives, and computes the
@@ -23,6 +25,8 @@
 #pragma once
 #include "hydro_kernels_basic.cuh"
 
+// blocks per SM the register cap of __launch_bounds__ is set for: fp32 one cell per thread (two 256-thread blocks,
+// <= 128 registers), and the two-rows-per-thread shape (one block)
 #ifndef PH_RPT2_MINB
 #define PH_RPT2_MINB 1
 #endif
