@@ -409,9 +409,14 @@ def sweep(binding, torch, args, peak, peak_src):
         w = make_workload(cfg)
         big = w.cells >= (1 << 22)
         steps = min(DEFAULT_STEPS[cfg], 100 if not big else 10)
-        for variant in ("fused", "march", "fused1", "manifest_flux", "manifest_all", "delayed"):
+        for variant in ("fused", "march", "fused1", "manifest_flux", "manifest_all", "delayed", "march arith=1"):
+            opts = None
+            if variant == "march arith=1":  # fp32 only: hardware rcp / rsqrt approximations, inside the tolerances, not bit-equal
+                if w.dtype != np.float32 or w.dims == 1:
+                    continue
+                opts = {"arith": 1}
             try:
-                r = device_run(binding, torch, w, steps, 3, variant, args.riemann, big)
+                r = device_run(binding, torch, w, steps, 3, variant.split()[0], args.riemann, big, opts)
             except Exception as ex:  # e.g. out of memory for manifest_all
                 out.append({"config": cfg, "variant": variant, "error": str(ex)[:120]})
                 continue

@@ -74,6 +74,9 @@ int paraiso_hydro_destroy(paraiso_hydro_t *h);
  *               (3-D), block_z = rows per main thread (3-D: 1 or 2), cells_per_thread 2 = packed f32x2;
  *               tile_depth = planes marched per block
  *   "graph"     1 replay steps of run() from a captured CUDA graph (default) | 0 plain launches
+ *   "arith"     k_march, fp32 only: 0 IEEE-exact division and square root, bit-equal to the oracle (default) |
+ *               1 hardware reciprocal / reciprocal-square-root approximations: inside north_star's fp32 tolerances,
+ *               not bit-equal, ~15 % faster (R21)
  *   "staging"   k_march only: 0 / 1 every thread loads its own cells (default) | 2 TMA bulk copies of the tile rows into a
  *               shared-memory ring (one cell per thread, n_x a multiple of 16 bytes; measured slower)
  *   "integrator" 0 the paper's two-stage midpoint rule, Eq. 24-27 (default) | 1 Heun / Shu-Osher SSP-RK2, the

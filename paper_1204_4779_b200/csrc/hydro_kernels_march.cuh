@@ -40,6 +40,11 @@ namespace ph {
 __device__ __forceinline__ float lane_first(float a) { return a; }
 __device__ __forceinline__ double lane_first(double a) { return a; }
 __device__ __forceinline__ float lane_first(f32x2 a) { return a.v.x; }
+__device__ __forceinline__ float lane_first(f32fast a) { return a.v; }
+__device__ __forceinline__ float lane_last(f32fast a) { return a.v; }
+__device__ __forceinline__ f32fast xshift_left(f32fast, float nb) { return f32fast(nb); }
+__device__ __forceinline__ f32fast xshift_right(f32fast, float nb) { return f32fast(nb); }
+__device__ __forceinline__ f32fast lane_pack(float a, float, f32fast*) { return f32fast(a); }
 __device__ __forceinline__ float lane_last(float a) { return a; }
 __device__ __forceinline__ double lane_last(double a) { return a; }
 __device__ __forceinline__ float lane_last(f32x2 a) { return a.v.y; }
@@ -58,6 +63,7 @@ __device__ __forceinline__ f32x2 lane_pack(float a, float b, f32x2*) { return f3
 template <class T> __device__ __forceinline__ T lds(const scalar_t<T>* p) { return *p; }
 template <> __device__ __forceinline__ f32x2 lds<f32x2>(const float* p) { return f32x2(*reinterpret_cast<const float2*>(p)); }
 __device__ __forceinline__ void sts(float* p, float v) { *p = v; }
+__device__ __forceinline__ void sts(float* p, f32fast v) { *p = v.v; }
 __device__ __forceinline__ void sts(double* p, double v) { *p = v; }
 __device__ __forceinline__ void sts(float* p, f32x2 v) { *reinterpret_cast<float2*>(p) = v.v; }
 
@@ -167,9 +173,12 @@ __device__ __forceinline__ T ld_cells_rw(const scalar_t<T>* A, int idx) {
   if constexpr (LaneTraits<T>::W == 1) return A[idx];
   else return f32x2(*reinterpret_cast<const float2*>(A + idx));
 }
+__device__ __forceinline__ float scalar_of(float v) { return v; }
+__device__ __forceinline__ double scalar_of(double v) { return v; }
+__device__ __forceinline__ float scalar_of(f32fast v) { return v.v; }
 template <class T>
 __device__ __forceinline__ void st_cells(scalar_t<T>* A, int idx, T v) {
-  if constexpr (LaneTraits<T>::W == 1) A[idx] = v;
+  if constexpr (LaneTraits<T>::W == 1) A[idx] = scalar_of(v);
   else *reinterpret_cast<float2*>(A + idx) = v.v;
 }
 __device__ __forceinline__ float shfl_dn(float v) { return __shfl_down_sync(0xffffffffu, v, 1); }
@@ -683,11 +692,13 @@ inline int march_default_depth(long long tiles_in_plane, int nM) {
 //         DESIGN.md §7)
 //   block[0] (2-D): main warps per block (0 = default); block[1] (3-D): main warps TY (0 = default);
 //   block[2] (3-D): rows per thread (0 / 1, or 2 with TY = 7)
+//   arith: 1 = fp32 with the hardware reciprocal / reciprocal square root approximations (f32fast: inside north_star's
+//          tolerances, not bit-equal to the oracle; default shapes only), 0 = IEEE-exact (default)
 //   staging: 0 / 1 = every thread loads its own cells (LDG), 2 = TMA bulk copies of the tile rows into a shared-memory
 //            ring (one cell per thread, n_x a multiple of 16 bytes, default tile shapes only)
 template <class Real, int D, int RS, int STAGE>
 bool launch_march_stage(const Real* Uin, const Real* Ubase, Real* Uout, const Geom<Real>& g, Scalars* sc,
-                        cudaStream_t stream, const int* block, int tile_depth, int pack, int staging) {
+                        cudaStream_t stream, const int* block, int tile_depth, int pack, int staging, int arith) {
   if constexpr (D == 1) {
     return false;
   } else {
@@ -707,6 +718,8 @@ bool launch_march_stage(const Real* Uin, const Real* Ubase, Real* Uout, const Ge
       if (packed) return launch_march_shape<f32x2, D, RS, STAGE, NWXV, 1, 1>(Uin, Ubase, Uout, g, sc, stream, depth); \
     return launch_march_shape<Real, D, RS, STAGE, NWXV, 1, minb>(Uin, Ubase, Uout, g, sc, stream, depth);           \
   }
+      if constexpr (can_pack)
+        if (arith == 1 && nwx == 4) return launch_march_shape<f32fast, D, RS, STAGE, 4, 1, minb>(Uin, Ubase, Uout, g, sc, stream, depth);
       if (tma && nwx == 4) return launch_march_shape<Real, D, RS, STAGE, 4, 1, minb, true>(Uin, Ubase, Uout, g, sc, stream, depth);
       PH_SHAPE(2) PH_SHAPE(3) PH_SHAPE(4) PH_SHAPE(7) PH_SHAPE(8)
 #undef PH_SHAPE
@@ -721,6 +734,8 @@ bool launch_march_stage(const Real* Uin, const Real* Ubase, Real* Uout, const Ge
       if (packed) return launch_march_shape<f32x2, D, RS, STAGE, 1, TYV, 1>(Uin, Ubase, Uout, g, sc, stream, depth);  \
     return launch_march_shape<Real, D, RS, STAGE, 1, TYV, (TYV > 8 ? 1 : minb)>(Uin, Ubase, Uout, g, sc, stream, depth);            \
   }
+      if constexpr (can_pack)
+        if (arith == 1 && ty == 7) return launch_march_shape<f32fast, D, RS, STAGE, 1, 7, minb>(Uin, Ubase, Uout, g, sc, stream, depth);
       if (tma && ty == 7) return launch_march_shape<Real, D, RS, STAGE, 1, 7, minb, true>(Uin, Ubase, Uout, g, sc, stream, depth);
       if (block[2] == 2 && ty == 7 && !packed)  // two rows per thread: a 32 x 14 tile, one 256-thread block per SM
         return launch_march_shape<Real, D, RS, STAGE, 1, 7, PH_RPT2_MINB, false, 2>(Uin, Ubase, Uout, g, sc, stream, depth);

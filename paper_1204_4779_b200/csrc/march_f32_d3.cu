@@ -5,7 +5,7 @@
 namespace ph {
 #define PH_INST(RS, STAGE)                                                                                         \
   template bool launch_march_stage<float, 3, RS, STAGE>(const float*, const float*, float*, const Geom<float>&, \
-                                                          Scalars*, cudaStream_t, const int*, int, int, int);
+                                                          Scalars*, cudaStream_t, const int*, int, int, int, int);
 PH_INST(RIEMANN_HLLC, 1)
 PH_INST(RIEMANN_HLLC, 2)
 PH_INST(RIEMANN_HLL, 1)

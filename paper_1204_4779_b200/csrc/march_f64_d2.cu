@@ -5,7 +5,7 @@
 namespace ph {
 #define PH_INST(RS, STAGE)                                                                                         \
   template bool launch_march_stage<double, 2, RS, STAGE>(const double*, const double*, double*, const Geom<double>&, \
-                                                          Scalars*, cudaStream_t, const int*, int, int, int);
+                                                          Scalars*, cudaStream_t, const int*, int, int, int, int);
 PH_INST(RIEMANN_HLLC, 1)
 PH_INST(RIEMANN_HLLC, 2)
 PH_INST(RIEMANN_HLL, 1)

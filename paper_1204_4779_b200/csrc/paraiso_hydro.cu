@@ -21,7 +21,7 @@ namespace ph {
   extern template bool launch_fused_stage<REAL, DD, RS, ST>(const REAL*, const REAL*, REAL*, const Geom<REAL>&, \
                                                             Scalars*, cudaStream_t, const int*, int);            \
   extern template bool launch_march_stage<REAL, DD, RS, ST>(const REAL*, const REAL*, REAL*, const Geom<REAL>&, \
-                                                            Scalars*, cudaStream_t, const int*, int, int, int);
+                                                            Scalars*, cudaStream_t, const int*, int, int, int, int);
 #define PH_EXTERN(REAL, DD)              \
   PH_EXTERN1(REAL, DD, RIEMANN_HLLC, 1)  \
   PH_EXTERN1(REAL, DD, RIEMANN_HLLC, 2)  \
@@ -49,6 +49,7 @@ struct paraiso_hydro {
   int boundary = BOUNDARY_PERIODIC, riemann = RIEMANN_HLLC, variant = VARIANT_FUSED;
   int block[3] = {0, 0, 0};
   int tile_depth = 0, cells_per_thread = 0, use_graph = 1;
+  int arith = 0;       // k_march fp32: 0 IEEE-exact division / square root, 1 hardware approximations (f32fast)
   int staging = 0;     // k_march: 0 / 1 own-cell LDG, 2 TMA bulk copies into a shared-memory ring
   int integrator = 0;  // 0 midpoint (paper) | 1 Heun
   int state_kind = 0;  // 0: set_state / get_state exchange conserved variables, 1: primitive variables
@@ -253,7 +254,7 @@ struct Launch {
       case VARIANT_MARCH:
         if ((h->variant == VARIANT_MARCH || D == 3 || sizeof(Real) == 4) &&
             launch_march_stage<Real, D, RS, STAGE>(Uin, stage_base<STAGE>(h), Uout, g, h->sc, h->stream, h->block,
-                                                   h->tile_depth, h->cells_per_thread, h->staging)) {
+                                                   h->tile_depth, h->cells_per_thread, h->staging, h->arith)) {
           h->launches += 1;
           break;
         }
@@ -342,6 +343,7 @@ static int options_key(const paraiso_hydro* h) {
   k = k * 1031 + h->tile_depth;
   k = k * 1031 + h->cells_per_thread;
   k = k * 7 + h->staging;
+  k = k * 3 + h->arith;
   return k & 0x7fffffff;
 }
 
@@ -432,7 +434,8 @@ static bool find_option(paraiso_hydro* h, const char* key, OptionRef* ref) {
                       {"graph", {&h->use_graph, 0, 1}},
                       {"state_kind", {&h->state_kind, 0, 1}},
                       {"integrator", {&h->integrator, 0, 1}},
-                      {"staging", {&h->staging, 0, 2}}};
+                      {"staging", {&h->staging, 0, 2}},
+                      {"arith", {&h->arith, 0, 1}}};
   for (const Opt& o : opts)
     if (!std::strcmp(key, o.key)) {
       *ref = o.ref;

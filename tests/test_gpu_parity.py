@@ -345,3 +345,27 @@ def test_march_two_rows_per_thread_matches_oracle(gpu, oracle_mod, shape, bounda
             got, gdt = gpu_steps(gpu, w, 3, "march", block_z=2, tile_depth=depth)
             assert np.array_equal(got, ref), (shape, dtype, depth, field_errors(got, ref))
             assert all(abs(a - b) <= TOL[np.dtype(dtype)][2] * b for a, b in zip(gdt, rdt))
+
+
+@pytest.mark.parametrize("boundary", ["periodic", "outflow"])
+@pytest.mark.parametrize("dims", [2, 3])
+def test_fast_arithmetic_option_stays_inside_the_tolerances(gpu, oracle_mod, dims, boundary):
+    """Option arith = 1 (fp32 with the hardware reciprocal / rsqrt approximations): not bit-equal to the oracle by
+    construction; north_star's fp32 tolerances (1e-5 one step, 1e-3 after 100, dt 1e-6) must hold."""
+    shape = {2: (203, 77), 3: (45, 38, 27)}[dims]
+    w = inputs.random_smooth(shape, np.float32, seed=61 + dims, boundary=boundary)
+    tol1, tol100, toldt = TOL[np.dtype(np.float32)]
+    for nsteps, tol in ((1, tol1), (100, tol100)):
+        ref, rdt = oracle_steps(oracle_mod, w, nsteps)
+        got, gdt = gpu_steps(gpu, w, nsteps, "march", arith=1)
+        err = field_errors(got, ref)
+        assert np.all(err <= tol), (nsteps, err)
+        assert all(abs(a - b) <= toldt * b for a, b in zip(gdt[:3], rdt[:3]))
+        assert not np.array_equal(got, ref)  # the option really is the approximate path
+
+
+def test_fast_arithmetic_option_on_kelvin_helmholtz(gpu, oracle_mod):
+    w = inputs.kelvin_helmholtz(256, dtype=np.float32, seed=0, steps=100)  # config 1's recipe at 256^2
+    ref, _ = oracle_steps(oracle_mod, w, 100)
+    got, _ = gpu_steps(gpu, w, 100, "march", arith=1)
+    assert np.all(field_errors(got, ref) <= 1e-3), field_errors(got, ref)
