@@ -416,7 +416,7 @@ def sweep(binding, torch, args, peak, peak_src):
                     continue
                 opts = {"arith": 1}
             try:
-                r = device_run(binding, torch, w, steps, 3, variant.split()[0], args.riemann, big, opts)
+                r = device_run(binding, torch, w, steps, 3 if w.cells >= (1 << 26) else 20, variant.split()[0], args.riemann, big, opts)
             except Exception as ex:  # e.g. out of memory for manifest_all
                 out.append({"config": cfg, "variant": variant, "error": str(ex)[:120]})
                 continue
