@@ -21,7 +21,7 @@ PARAISO_OK, PARAISO_EINVAL, PARAISO_ENOMEM, PARAISO_ECUDA, PARAISO_ESTATE, PARAI
 
 BOUNDARY = {"periodic": 0, "outflow": 1}
 RIEMANN = {"hllc": 0, "hll": 1}
-VARIANT = {"fused": 0, "manifest_flux": 1, "manifest_all": 2, "delayed": 3, "march": 4, "fused1": 5}
+VARIANT = {"fused": 0, "manifest_flux": 1, "manifest_all": 2, "delayed": 3, "march": 4, "fused1": 5, "pack": 6}
 
 _vp, _i64, _dbl, _int = ctypes.c_void_p, ctypes.c_int64, ctypes.c_double, ctypes.c_int
 _pi64, _pdbl = ctypes.POINTER(_i64), ctypes.POINTER(_dbl)

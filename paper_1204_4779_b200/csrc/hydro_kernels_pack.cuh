@@ -1,0 +1,496 @@
+// hydro_kernels_pack.cuh — the fused RK-stage kernel, third design ("pack"): fp32, TWO x-adjacent cells per thread on
+// the packed sm_100 instructions FADD2 / FMUL2 / FFMA2, built so that the packed arithmetic fits 128 registers and
+// sixteen warps per SM (profiles/r2_README.md: the r1 packed kernel needed 213 registers, two warps per scheduler,
+// and lost to the scalar kernel for that reason alone).
+//
+// Same tile / marching scheme as k_march (hydro_kernels_march.cuh): a block = TY main warps, one row of 64 cells each
+// (3-D; in 2-D NWX warps side by side on one row), plus ONE halo warp; the tile is marched through `depth` planes of
+// the last axis; every primitive recovery, slope and Riemann solve of a cell / face is done once (Fig. 6-7
+// :435-472, "Manifest in SRAM").  What differs:
+//   * the rolling window along the marching axis does not live in registers.  The primitives of planes m, m+1, m+2
+//     sit in a ring of three shared-memory planes (plane m with its 2-cell star halo); the high-side state of plane m
+//     and the flux through face m-1/2 sit in per-thread shared-memory slots.  No register rotates at the loop edge.
+//   * x-neighbours exchange by warp shuffle at once (before the barrier); only the y direction and the warp-edge
+//     lanes wait for a block barrier.
+// Arithmetic: DESIGN.md §4 through the lane-generic functions of hydro_math.cuh with T = f32x2, bit-identical per
+// lane to the scalar kernels and to the oracle (tests/test_gpu_parity.py).  n_x must be even (pairs are 8-byte
+// aligned and wrap as pairs); the launcher falls back to k_march otherwise.
+#pragma once
+#include "hydro_kernels_march.cuh"
+
+namespace ph {
+
+template <int D, int NWX, int TY>
+struct PackShape {
+  using T = f32x2;
+  static constexpr int NF = D + 2;
+  static constexpr int TXC = NWX * 64;                   // cells per tile row
+  static constexpr int PX = TXC + 4;                     // plane row: tile + 2 halo cells on each side
+  static constexpr int PY = (D == 3) ? TY + 4 : 1;
+  static constexpr int OY = (D == 3) ? 2 : 0;
+  static constexpr int NMAIN = NWX * TY * 32;
+  static constexpr int NT = NMAIN + 32;
+  static constexpr int XROWS = (D == 3) ? TY : 1;
+  static_assert(D == 2 || D == 3, "2-D and 3-D grids");
+  static_assert(D == 3 || TY == 1, "2-D tiles are rows");
+  static_assert(D == 2 || NWX == 1, "3-D tiles are one warp wide");
+  static_assert(XROWS <= 64, "tile too tall for one halo warp");
+  struct Smem {
+    float V[3][NF][PY][PX];                               // ring: primitives of planes m (with halo), m+1, m+2
+    float Hm[NF][XROWS][TXC];                             // high-side marching-axis state of plane m, own cells
+    float Fp[NF][XROWS][TXC];                             // flux through the marching-axis face m-1/2, own cells
+    float LOy[(D == 3) ? NF : 1][XROWS + 1][(D == 3) ? TXC : 2];  // [r]: low-side y state of tile row r (r = TY: halo warp)
+    float Fy[(D == 3) ? NF : 1][XROWS][(D == 3) ? TXC : 2];       // [r]: flux through the low y face of row r (r = 0: halo warp)
+    float Un[NF][XROWS][TXC];                             // cp.async staging: U_in of plane m+2, own cells
+    float Ub[NF][XROWS][TXC];                             // cp.async staging: U_base of plane m, own cells
+    float LOx[NF][XROWS][NWX + 1];                        // [e]: low-side x state of the first cell of warp column e
+    float Fx[NF][XROWS][NWX];                             // [e]: flux through the low x face of warp column e
+  };
+};
+
+// 8-byte asynchronous copy global -> shared of one pair of cells (cp.async: SASS LDGSTS), read back by the issuing
+// thread after cp_async_wait_all(): no register is held while the load is in flight
+__device__ __forceinline__ void cp_async8(float* dst_smem, const float* src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_addr(dst_smem)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async4(float* dst_smem, const float* src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_addr(dst_smem)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+// BND: the boundary mode as a compile-time constant.  On periodic grids (n_x even) every pair of cells a thread
+// touches, ghost pairs included, is one aligned 8-byte pair in memory; outflow ghosts are clamped cell by cell.
+template <int D, int RS, int STAGE, int NWX, int TY, int MINB, int BND>
+__global__ void __launch_bounds__(PackShape<D, NWX, TY>::NT, MINB)
+    k_pack(const float* __restrict__ Uin, const float* Ubase, float* Uout, Geom<float> g, Scalars* sc, int depth) {
+  using Sh = PackShape<D, NWX, TY>;
+  using T = f32x2;
+  using P = Prim<T, D>;
+  constexpr int NF = Sh::NF, TXC = Sh::TXC, OY = Sh::OY, XROWS = Sh::XROWS;
+  constexpr int M = D - 1;  // marching axis
+  constexpr int W = 2;
+
+  if (sc->done) return;
+  extern __shared__ __align__(128) unsigned char pack_smem_raw[];
+  typename Sh::Smem& sm = *reinterpret_cast<typename Sh::Smem*>(pack_smem_raw);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int nx = g.n[0], ny = g.n[1], nM = g.n[M];
+  constexpr int bnd = BND;
+  const int x0 = blockIdx.x * TXC;
+  const int y0 = (D == 3) ? blockIdx.y * TY : 0;
+  const int bm = (D == 3) ? blockIdx.z : blockIdx.y;
+  const int m0 = bm * depth;
+  const int m1 = min(m0 + depth, nM);
+  const int Ni = int(g.N);
+  const int psi = (D == 3) ? nx * ny : nx;
+  auto plane_of = [&](int m) { return map_index(m, nM, bnd) * psi; };
+  auto grid_row = [&](int gj) { return (D == 3) ? march_src(gj, ny, bnd) * nx : 0; };
+  // the W cells of a CellSrc: one 8-byte load when they are known to be a pair
+  auto ldg_pair = [&](const float* __restrict__ A, int base, const CellSrc& c) {
+    if constexpr (BND == BOUNDARY_PERIODIC) return f32x2(__ldg(reinterpret_cast<const float2*>(A + (base + c.o0))));
+    else return ldg_cells<T>(A, base, c);
+  };
+
+  float s_max = 0.0f;
+  int bad = 0;
+
+  if (warp < NWX * TY) {
+    // =========================================================================== main warps
+    const int wx = (D == 3) ? 0 : warp;
+    const int row = (D == 3) ? warp : 0;
+    const int c0 = (wx * 32 + lane) * W;  // first own cell, tile coordinates
+    const int gi = x0 + c0;
+    const int gj = y0 + row;
+    const int pc = c0 + 2, pr = row + OY;
+    const bool active = gi < nx && (D == 2 || gj < ny);
+    const CellSrc src = cell_src<T>(gi, grid_row(gj), nx, bnd);
+    const int own = (D == 3 ? gj * nx : 0) + gi;
+
+    auto load_cells_of = [&](int m, T (&u)[NF]) {
+      const int pl = plane_of(m);
+#pragma unroll
+      for (int f = 0; f < NF; ++f) u[f] = ldg_pair(Uin, f * Ni + pl, src);
+    };
+    // asynchronous copies into this thread's staging slots: U_in of plane mi (own cells) and, when cell >= 0, the
+    // own-cell U_base of the plane being updated
+    auto stage_copies = [&](int mi, int cell) {
+      const int pl = plane_of(mi);
+#pragma unroll
+      for (int f = 0; f < NF; ++f) {
+        if constexpr (BND == BOUNDARY_PERIODIC) {
+          cp_async8(&sm.Un[f][row][c0], Uin + (f * Ni + pl + src.o0));
+        } else {
+          cp_async4(&sm.Un[f][row][c0], Uin + (f * Ni + pl + src.o0));
+          cp_async4(&sm.Un[f][row][c0 + 1], Uin + (f * Ni + pl + src.o1));
+        }
+        if (active && cell >= 0) cp_async8(&sm.Ub[f][row][c0], Ubase + (f * Ni + cell));
+      }
+    };
+    const float lam0 = float(sc->lam[STAGE - 1][0]);
+    const float lam1 = float(sc->lam[STAGE - 1][1]);
+    const float lam2 = (D == 3) ? float(sc->lam[STAGE - 1][2]) : 0.0f;
+
+    // ---- prologue: planes m0, m0+1 of the ring, the high-side state of plane m0 and the flux through face m0-1/2
+    {
+      T u[NF];
+      load_cells_of(m0 - 2, u);
+      const P Vm2 = prim_of<T, D>(u, g.gm1);
+      load_cells_of(m0 - 1, u);
+      const P Vm1 = prim_of<T, D>(u, g.gm1);
+      load_cells_of(m0, u);
+      const P Vc = prim_of<T, D>(u, g.gm1);
+      load_cells_of(m0 + 1, u);
+      const P Vp1 = prim_of<T, D>(u, g.gm1);
+      P him1, loc, hiM;
+      interpolate<T, D>(Vm2, Vm1, Vc, nullptr, &him1);
+      interpolate<T, D>(Vm1, Vc, Vp1, &loc, &hiM);
+      T F[NF], a[NF];
+      riemann_flux<T, D, M, RS>(g.gamma, g.igm1, him1, loc, F);
+      prim_to_fields<T, D>(Vc, a);
+#pragma unroll
+      for (int f = 0; f < NF; ++f) sts(&sm.V[0][f][pr][pc], a[f]);
+      prim_to_fields<T, D>(Vp1, a);
+#pragma unroll
+      for (int f = 0; f < NF; ++f) sts(&sm.V[1][f][pr][pc], a[f]);
+      prim_to_fields<T, D>(hiM, a);
+#pragma unroll
+      for (int f = 0; f < NF; ++f) {
+        sts(&sm.Hm[f][row][c0], a[f]);
+        sts(&sm.Fp[f][row][c0], F[f]);
+      }
+    }
+    stage_copies(m0 + 2, -1);
+    block_barrier();
+
+    int s0 = 0, s1 = 1, s2 = 2;  // ring slots of planes m, m+1, m+2
+    for (int m = m0; m < m1; ++m) {
+      // ------------------------------------------------------------ phase A
+      const int cell = plane_of(m) + own;
+      T vc[NF];
+#pragma unroll
+      for (int f = 0; f < NF; ++f) vc[f] = lds<T>(&sm.V[s0][f][pr][pc]);
+      // marching axis: V[m+2] (its U_in was copied during the previous iteration), slope of cell m+1, flux through
+      // face m+1/2; then the copies of U_in of plane m+3 (next iteration) and of the own-cell U_base of plane m (phase C)
+      T dFm[NF];
+      {
+        cp_async_wait_all();
+        T un[NF];
+#pragma unroll
+        for (int f = 0; f < NF; ++f) un[f] = lds<T>(&sm.Un[f][row][c0]);
+        stage_copies(m + 3, cell);
+        const P Vp2 = prim_of<T, D>(un, g.gm1);
+        T vp2[NF], loM1[NF], hiM[NF];
+        prim_to_fields<T, D>(Vp2, vp2);
+#pragma unroll
+        for (int f = 0; f < NF; ++f) {
+          sts(&sm.V[s2][f][pr][pc], vp2[f]);
+          const T vp1 = lds<T>(&sm.V[s1][f][pr][pc]);
+          const T dy = minbee_dy(vc[f], vp1, vp2[f]);
+          loM1[f] = rfma(-0.5f, dy, vp1);
+          hiM[f] = lds<T>(&sm.Hm[f][row][c0]);
+          sts(&sm.Hm[f][row][c0], rfma(0.5f, dy, vp1));
+        }
+        T Fn[NF];
+        riemann_flux<T, D, M, RS>(g.gamma, g.igm1, prim_from_fields<T, D>(hiM), prim_from_fields<T, D>(loM1), Fn);
+#pragma unroll
+        for (int f = 0; f < NF; ++f) {
+          dFm[f] = lds<T>(&sm.Fp[f][row][c0]) - Fn[f];
+          sts(&sm.Fp[f][row][c0], Fn[f]);
+        }
+      }
+      // x slopes; the low-side state goes to the left neighbour at once (shuffle), lane 31 is patched after the barrier
+      T hix[NF], rs[NF];
+#pragma unroll
+      for (int f = 0; f < NF; ++f) {
+        const T l = xshift_left(vc[f], sm.V[s0][f][pr][pc - 1]);
+        const T r = xshift_right(vc[f], sm.V[s0][f][pr][pc + W]);
+        const T dy = minbee_dy(l, vc[f], r);
+        const T lox = rfma(-0.5f, dy, vc[f]);
+        hix[f] = rfma(0.5f, dy, vc[f]);
+        if (lane == 0) sm.LOx[f][row][wx] = lox.v.x;
+        rs[f] = xshift_right(lox, shfl_dn(lox.v.x));
+      }
+      T hiy[(D == 3) ? NF : 1];
+      if constexpr (D == 3) {
+#pragma unroll
+        for (int f = 0; f < NF; ++f) {
+          const T dy = minbee_dy(lds<T>(&sm.V[s0][f][pr - 1][pc]), vc[f], lds<T>(&sm.V[s0][f][pr + 1][pc]));
+          sts(&sm.LOy[f][row][c0], rfma(-0.5f, dy, vc[f]));
+          hiy[f] = rfma(0.5f, dy, vc[f]);
+        }
+      }
+      block_barrier();
+
+      // ------------------------------------------------------------ phase B: one Riemann solve per in-plane face
+      T Fx[NF], Fy[(D == 3) ? NF : 1];
+      if (lane == 31) {
+#pragma unroll
+        for (int f = 0; f < NF; ++f) rs[f].v.y = sm.LOx[f][row][wx + 1];
+      }
+      riemann_flux<T, D, 0, RS>(g.gamma, g.igm1, prim_from_fields<T, D>(hix), prim_from_fields<T, D>(rs), Fx);
+      if (NWX > 1 && lane == 31 && wx + 1 < NWX) {
+#pragma unroll
+        for (int f = 0; f < NF; ++f) sm.Fx[f][row][wx + 1] = Fx[f].v.y;
+      }
+      if constexpr (D == 3) {
+        T a[NF];
+#pragma unroll
+        for (int f = 0; f < NF; ++f) a[f] = lds<T>(&sm.LOy[f][row + 1][c0]);
+        riemann_flux<T, D, 1, RS>(g.gamma, g.igm1, prim_from_fields<T, D>(hiy), prim_from_fields<T, D>(a), Fy);
+        if (row + 1 < TY) {
+#pragma unroll
+          for (int f = 0; f < NF; ++f) sts(&sm.Fy[f][row + 1][c0], Fy[f]);
+        }
+      }
+      block_barrier();
+
+      // ------------------------------------------------------------ phase C: Eq. 23, axes in the order x, y, z
+      T lowx[NF];
+#pragma unroll
+      for (int f = 0; f < NF; ++f) {
+        float nb = shfl_up(Fx[f].v.y);
+        if (lane == 0) nb = sm.Fx[f][row][wx];
+        lowx[f] = xshift_left(Fx[f], nb);
+      }
+      cp_async_wait_all();
+      if (active) {
+        T u[NF];  // own-cell base state of Eq. 23 (copied in phase A; U_base is overwritten in place only below)
+#pragma unroll
+        for (int f = 0; f < NF; ++f) u[f] = rfma(lam0, lowx[f] - Fx[f], lds<T>(&sm.Ub[f][row][c0]));
+        if constexpr (D == 3) {
+#pragma unroll
+          for (int f = 0; f < NF; ++f) u[f] = rfma(lam1, lds<T>(&sm.Fy[f][row][c0]) - Fy[f], u[f]);
+#pragma unroll
+          for (int f = 0; f < NF; ++f) u[f] = rfma(lam2, dFm[f], u[f]);
+        } else {
+#pragma unroll
+          for (int f = 0; f < NF; ++f) u[f] = rfma(lam1, dFm[f], u[f]);
+        }
+        if (STAGE == 2 && g.integrator == 1) {  // Heun: U2 = 0.5 (U0 + (U1 + dt L(U1))); U0 still sits in Uout
+#pragma unroll
+          for (int f = 0; f < NF; ++f) u[f] = 0.5f * (ld_cells_rw<T>(Uout, f * Ni + cell) + u[f]);
+        }
+#pragma unroll
+        for (int f = 0; f < NF; ++f) st_cells<T>(Uout, f * Ni + cell, u[f]);
+        if (STAGE == 2) {
+          T ir;
+          const P Vn = prim_of<T, D>(u, g.gm1, &ir);
+          s_max = rmax(s_max, lane_max(cfl_speed<T, D>(Vn, ir, g.gamma, g.idr)));
+          bad += bad_lanes<T, D>(Vn, u[NF - 1]);
+        }
+      }
+      const int t = s0;
+      s0 = s1;
+      s1 = s2;
+      s2 = t;
+    }
+  } else {
+    // =========================================================================== the halo warp
+    // Loads the 2-cell star halo of every plane, converts it to primitives (into the ring slot of the NEXT plane) and
+    // computes the faces the tile cannot get from its own cells.
+    constexpr int XHALO = 2 * XROWS;                    // x halo pairs per plane: rows x {left pair, right pair}
+    constexpr int NXP = (XHALO + 31) / 32;
+    CellSrc hsrc[NXP];
+    int hpy[NXP], hpx[NXP];
+    bool hval[NXP];
+#pragma unroll
+    for (int q = 0; q < NXP; ++q) {
+      const int id = lane + 32 * q;
+      hval[q] = id < XHALO;
+      const int r = hval[q] ? (id >> 1) : 0;
+      const int px = (id & 1) ? TXC + 2 : 0;
+      hpy[q] = r + OY;
+      hpx[q] = px;
+      hsrc[q] = cell_src<T>(x0 + px - 2, grid_row(y0 + r), nx, bnd);
+    }
+    constexpr int NYP = (D == 3) ? 4 : 0;  // y halo rows
+    CellSrc ysrc[NYP > 0 ? NYP : 1];
+#pragma unroll
+    for (int q = 0; q < NYP; ++q) ysrc[q] = cell_src<T>(x0 + lane * W, grid_row(y0 + (q < 2 ? q : TY + q) - 2), nx, bnd);
+    T Uh[NXP][NF], Uyh[NYP > 0 ? NYP : 1][NF];
+    auto load_halo = [&](int m) {
+      const int pl = plane_of(m);
+#pragma unroll
+      for (int q = 0; q < NXP; ++q)
+        if (hval[q]) {
+#pragma unroll
+          for (int f = 0; f < NF; ++f) Uh[q][f] = ldg_pair(Uin, f * Ni + pl, hsrc[q]);
+        }
+#pragma unroll
+      for (int q = 0; q < NYP; ++q) {
+#pragma unroll
+        for (int f = 0; f < NF; ++f) Uyh[q][f] = ldg_pair(Uin, f * Ni + pl, ysrc[q]);
+      }
+    };
+    auto store_halo = [&](int s) {
+      T u[NF];
+#pragma unroll
+      for (int q = 0; q < NXP; ++q)
+        if (hval[q]) {
+          prim_to_fields<T, D>(prim_of<T, D>(Uh[q], g.gm1), u);
+#pragma unroll
+          for (int f = 0; f < NF; ++f) sts(&sm.V[s][f][hpy[q]][hpx[q]], u[f]);
+        }
+#pragma unroll
+      for (int q = 0; q < NYP; ++q) {
+        prim_to_fields<T, D>(prim_of<T, D>(Uyh[q], g.gm1), u);
+#pragma unroll
+        for (int f = 0; f < NF; ++f) sts(&sm.V[s][f][q < 2 ? q : TY + q][lane * W + 2], u[f]);
+      }
+    };
+    // x face tasks: lane l handles tile rows ra (first lane of T) and rb (second lane)
+    constexpr int XTASK_LANES = (XROWS + 1) / 2;
+    const bool xtask = lane < XTASK_LANES;
+    const int ra = xtask ? lane : 0;
+    const int rb = min(ra + XTASK_LANES, XROWS - 1);
+    auto plane_x = [&](int s, int qx) {
+      T u[NF];
+#pragma unroll
+      for (int f = 0; f < NF; ++f) u[f] = T(sm.V[s][f][ra + OY][qx], sm.V[s][f][rb + OY][qx]);
+      return prim_from_fields<T, D>(u);
+    };
+    auto plane_y = [&](int s, int py) {
+      T u[NF];
+#pragma unroll
+      for (int f = 0; f < NF; ++f) u[f] = lds<T>(&sm.V[s][f][py][lane * W + 2]);
+      return prim_from_fields<T, D>(u);
+    };
+
+    load_halo(m0);
+    store_halo(0);
+    if (m0 + 1 < m1) load_halo(m0 + 1);
+    block_barrier();
+
+    int s0 = 0, s1 = 1, s2 = 2;
+    for (int m = m0; m < m1; ++m) {
+      const bool more = m + 1 < m1;
+      // ---- phase A: high-side states of the cells just below the tile, low-side states of those just above;
+      //      primitives of the next plane's halo (loaded during the previous phase B)
+      P hiYlow, hiXlow;
+      if constexpr (D == 3) {
+        interpolate<T, D>(plane_y(s0, 0), plane_y(s0, 1), plane_y(s0, 2), nullptr, &hiYlow);
+        P lo;
+        interpolate<T, D>(plane_y(s0, TY + 1), plane_y(s0, TY + 2), plane_y(s0, TY + 3), &lo, nullptr);
+        T a[NF];
+        prim_to_fields<T, D>(lo, a);
+#pragma unroll
+        for (int f = 0; f < NF; ++f) sts(&sm.LOy[f][TY][lane * W], a[f]);
+      }
+      if (xtask) {
+        interpolate<T, D>(plane_x(s0, 0), plane_x(s0, 1), plane_x(s0, 2), nullptr, &hiXlow);
+        P lo;
+        interpolate<T, D>(plane_x(s0, TXC + 1), plane_x(s0, TXC + 2), plane_x(s0, TXC + 3), &lo, nullptr);
+        T a[NF];
+        prim_to_fields<T, D>(lo, a);
+#pragma unroll
+        for (int f = 0; f < NF; ++f) {
+          sm.LOx[f][ra][NWX] = a[f].v.x;
+          sm.LOx[f][rb][NWX] = a[f].v.y;
+        }
+      }
+      if (more) store_halo(s1);
+      block_barrier();
+      // ---- phase B: flux through the tile's low faces; loads of the halo of plane m+2
+      if constexpr (D == 3) {
+        T a[NF], F[NF];
+#pragma unroll
+        for (int f = 0; f < NF; ++f) a[f] = lds<T>(&sm.LOy[f][0][lane * W]);
+        riemann_flux<T, D, 1, RS>(g.gamma, g.igm1, hiYlow, prim_from_fields<T, D>(a), F);
+#pragma unroll
+        for (int f = 0; f < NF; ++f) sts(&sm.Fy[f][0][lane * W], F[f]);
+      }
+      if (xtask) {
+        T a[NF], F[NF];
+#pragma unroll
+        for (int f = 0; f < NF; ++f) a[f] = T(sm.LOx[f][ra][0], sm.LOx[f][rb][0]);
+        riemann_flux<T, D, 0, RS>(g.gamma, g.igm1, hiXlow, prim_from_fields<T, D>(a), F);
+#pragma unroll
+        for (int f = 0; f < NF; ++f) {
+          sm.Fx[f][ra][0] = F[f].v.x;
+          sm.Fx[f][rb][0] = F[f].v.y;
+        }
+      }
+      if (m + 2 < m1) load_halo(m + 2);
+      block_barrier();
+      const int t = s0;
+      s0 = s1;
+      s1 = s2;
+      s2 = t;
+    }
+  }
+  if (STAGE == 2) {
+    const unsigned int nblocks = gridDim.x * gridDim.y * gridDim.z;
+    block_reduce_and_finalize<float>(s_max, bad, sc, g, nblocks, 1);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+template <int D, int RS, int STAGE, int NWX, int TY, int MINB, int BND>
+static bool launch_pack_bnd(const float* Uin, const float* Ubase, float* Uout, const Geom<float>& g, Scalars* sc,
+                            cudaStream_t stream, int depth) {
+  using Sh = PackShape<D, NWX, TY>;
+  auto kern = k_pack<D, RS, STAGE, NWX, TY, MINB, BND>;
+  static bool configured[64] = {};
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return false;
+  if (!configured[dev]) {
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(typename Sh::Smem)) != cudaSuccess)
+      return false;
+    configured[dev] = true;
+  }
+  constexpr int M = D - 1;
+  dim3 grid, block(Sh::NT, 1, 1);
+  grid.x = (g.n[0] + Sh::TXC - 1) / Sh::TXC;
+  if (D == 3) {
+    grid.y = (g.n[1] + TY - 1) / TY;
+    grid.z = (g.n[M] + depth - 1) / depth;
+    if (grid.y > 65535u || grid.z > 65535u) return false;
+  } else {
+    grid.y = (g.n[M] + depth - 1) / depth;
+    grid.z = 1;
+    if (grid.y > 65535u) return false;
+  }
+  kern<<<grid, block, sizeof(typename Sh::Smem), stream>>>(Uin, Ubase, Uout, g, sc, depth);
+  return true;
+}
+
+template <int D, int RS, int STAGE, int NWX, int TY, int MINB>
+static bool launch_pack_shape(const float* Uin, const float* Ubase, float* Uout, const Geom<float>& g, Scalars* sc,
+                              cudaStream_t stream, int depth) {
+  if (g.boundary == BOUNDARY_PERIODIC)
+    return launch_pack_bnd<D, RS, STAGE, NWX, TY, MINB, BOUNDARY_PERIODIC>(Uin, Ubase, Uout, g, sc, stream, depth);
+  return launch_pack_bnd<D, RS, STAGE, NWX, TY, MINB, BOUNDARY_OUTFLOW>(Uin, Ubase, Uout, g, sc, stream, depth);
+}
+
+// Returns false when the packed kernel does not cover this shape (odd n_x, unknown block shape): the caller falls back.
+//   block[0] (2-D): main warps per block (0 = default); block[1] (3-D): main warps TY (0 = default)
+template <int D, int RS, int STAGE>
+bool launch_pack_stage(const float* Uin, const float* Ubase, float* Uout, const Geom<float>& g, Scalars* sc,
+                       cudaStream_t stream, const int* block, int tile_depth) {
+  if constexpr (D == 1) {
+    return false;
+  } else {
+    if (g.n[0] % 2 != 0) return false;
+    if constexpr (D == 2) {
+      const int nwx = block[0] > 0 ? block[0] : 4;
+      const long long tiles = (g.n[0] + nwx * 64 - 1) / (nwx * 64);
+      const int depth = tile_depth > 0 ? tile_depth : march_default_depth(tiles, g.n[1]);
+      if (nwx == 2) return launch_pack_shape<D, RS, STAGE, 2, 1, 2>(Uin, Ubase, Uout, g, sc, stream, depth);
+      if (nwx == 4) return launch_pack_shape<D, RS, STAGE, 4, 1, 2>(Uin, Ubase, Uout, g, sc, stream, depth);
+      if (nwx == 7) return launch_pack_shape<D, RS, STAGE, 7, 1, 2>(Uin, Ubase, Uout, g, sc, stream, depth);
+      return false;
+    } else {
+      const int ty = block[1] > 0 ? block[1] : 7;
+      const long long tiles = (long long)((g.n[0] + 63) / 64) * ((g.n[1] + ty - 1) / ty);
+      const int depth = tile_depth > 0 ? tile_depth : march_default_depth(tiles, g.n[2]);
+      if (ty == 7) return launch_pack_shape<D, RS, STAGE, 1, 7, 2>(Uin, Ubase, Uout, g, sc, stream, depth);
+      if (ty == 5) return launch_pack_shape<D, RS, STAGE, 1, 5, 2>(Uin, Ubase, Uout, g, sc, stream, depth);
+      if (ty == 11) return launch_pack_shape<D, RS, STAGE, 1, 11, 1>(Uin, Ubase, Uout, g, sc, stream, depth);
+      if (ty == 15) return launch_pack_shape<D, RS, STAGE, 1, 15, 1>(Uin, Ubase, Uout, g, sc, stream, depth);
+      return false;
+    }
+  }
+}
+
+}  // namespace ph

@@ -12,6 +12,7 @@
 #include "hydro_kernels_basic.cuh"
 #include "hydro_kernels_fused.cuh"
 #include "hydro_kernels_march.cuh"
+#include "hydro_kernels_pack.cuh"
 
 using namespace ph;
 
@@ -33,10 +34,17 @@ PH_EXTERN(double, 2)
 PH_EXTERN(double, 3)
 #undef PH_EXTERN
 #undef PH_EXTERN1
+// the packed fp32 kernels live in pack_f32_d<D>.cu
+#define PH_EXTERN_PACK(DD, RS, ST)                                                                             \
+  extern template bool launch_pack_stage<DD, RS, ST>(const float*, const float*, float*, const Geom<float>&, \
+                                                     Scalars*, cudaStream_t, const int*, int);
+PH_EXTERN_PACK(2, RIEMANN_HLLC, 1) PH_EXTERN_PACK(2, RIEMANN_HLLC, 2) PH_EXTERN_PACK(2, RIEMANN_HLL, 1) PH_EXTERN_PACK(2, RIEMANN_HLL, 2)
+PH_EXTERN_PACK(3, RIEMANN_HLLC, 1) PH_EXTERN_PACK(3, RIEMANN_HLLC, 2) PH_EXTERN_PACK(3, RIEMANN_HLL, 1) PH_EXTERN_PACK(3, RIEMANN_HLL, 2)
+#undef PH_EXTERN_PACK
 }  // namespace ph
 
 enum { VARIANT_FUSED = 0, VARIANT_MANIFEST_FLUX = 1, VARIANT_MANIFEST_ALL = 2, VARIANT_DELAYED = 3, VARIANT_MARCH = 4,
-       VARIANT_FUSED1 = 5 };
+       VARIANT_FUSED1 = 5, VARIANT_PACK = 6 };
 
 struct paraiso_hydro {
   int dims = 0, dtype = 0, nf = 0;
@@ -249,6 +257,15 @@ struct Launch {
         update<STAGE>(h, g, Uout);
         break;
       }
+      case VARIANT_PACK:
+        if constexpr (sizeof(Real) == 4 && D >= 2) {
+          if (launch_pack_stage<D, RS, STAGE>((const float*)Uin, (const float*)stage_base<STAGE>(h), (float*)Uout, g, h->sc,
+                                              h->stream, h->block, h->tile_depth)) {
+            h->launches += 1;
+            break;
+          }
+        }
+        // shapes the packed kernel does not cover (fp64, 1-D, odd n_x): the default on-chip kernel
       case VARIANT_FUSED:  // the faster of the two on-chip designs per grid kind (profiles/r1d_tune_*.txt):
                            // k_march in 3-D and in 2-D fp32, k_fused in 2-D fp64
       case VARIANT_MARCH:
@@ -425,7 +442,7 @@ static bool find_option(paraiso_hydro* h, const char* key, OptionRef* ref) {
   };
   const Opt opts[] = {{"boundary", {&h->boundary, 0, 1}},
                       {"riemann", {&h->riemann, 0, 1}},
-                      {"variant", {&h->variant, 0, 5}},
+                      {"variant", {&h->variant, 0, 6}},
                       {"block_x", {&h->block[0], 0, 1024}},
                       {"block_y", {&h->block[1], 0, 1024}},
                       {"block_z", {&h->block[2], 0, 64}},

@@ -13,7 +13,7 @@ from paper_1204_4779_b200 import inputs
 
 pytestmark = pytest.mark.gpu
 
-VARIANTS = ["fused", "march", "fused1", "manifest_flux", "manifest_all", "delayed"]
+VARIANTS = ["fused", "march", "fused1", "pack", "manifest_flux", "manifest_all", "delayed"]
 
 
 @pytest.fixture(scope="module")
