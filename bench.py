@@ -390,7 +390,7 @@ def main():
         # measured issue cost (scheduler cycles per instruction) of the instruction classes of the stage kernel on
         # this device: the model DESIGN.md §8 reads the ncu captures with
         mhz = (clocks or {}).get("sm_mhz") or 1965.0
-        line["roofline"]["issue_cost_cycles"] = {k: round(binding.debug_issue_cost(k, mhz)[0], 3) for k in binding.ISSUE_KINDS}
+        line["roofline"]["issue_cost_cycles"] = {k: round(binding.probe_issue_cost(k, mhz)[0], 3) for k in binding.ISSUE_KINDS}
     if rank == 0 and not args.no_sweep:
         line["all_configs"] = sweep(binding, torch, args, peak, peak_src)
     if rank == 0 and not args.no_cpu:

@@ -137,22 +137,6 @@ int paraiso_hydro_launch_count(paraiso_hydro_t *h, int64_t *launches);
  * Either pointer may be NULL. */
 int paraiso_hydro_kernel_time(paraiso_hydro_t *h, int enable, double *total_ms, int64_t *stage_launches);
 
-/* Test hook: evaluates the hot path's division and square root (DESIGN.md §4 "div_rn / sqrt_rn": the
- * fast path of the IEEE sequences without range check) element-wise on DEVICE arrays of n elements of
- * `dtype`: quot[i] = a[i] / b[i], root[i] = sqrt(|a[i]|).  Runs on the legacy default stream and
- * blocks.  Used by tests/test_gpu_arith.py to check correct rounding against IEEE over the normal range. */
-int paraiso_hydro_debug_arith(int dtype, int64_t n, const void *a, const void *b, void *quot, void *root);
-
-/* Measurement aid (csrc/microbench.cu): scheduler cycles that ONE more instruction of a class costs
- * next to 16 independent FFMA per loop iteration, 8 warps per scheduler, on the current device.
- *   kind 0 FFMA | 1 FMNMX | 2 FSETP+FSEL (per instruction of the pair) | 3 IADD3+LOP3 (per instruction) |
- *        4 FFMA2 (packed f32x2) | 5 DFMA | 6 MUFU.RCP
- * sm_clock_mhz: the SM clock to convert time into cycles with (the caller samples it, e.g. nvidia-smi clocks.sm).
- * base_cycles_per_iteration (may be NULL): cycles of the 16-FFMA loop alone.  Runs and synchronises on the
- * default stream.  EINVAL for an unknown kind, ECUDA / ENOMEM on failure. */
-int paraiso_hydro_debug_issue_cost(int kind, double sm_clock_mhz, double *cycles_per_instruction,
-                                   double *base_cycles_per_iteration);
-
 /* Message for the last error on this handle (or the last create failure when h == NULL).  Never NULL. */
 const char *paraiso_hydro_last_error(const paraiso_hydro_t *h);
 

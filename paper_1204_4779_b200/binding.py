@@ -43,13 +43,20 @@ SIGNATURES = {
     "paraiso_hydro_stats": (_int, [_vp, _pi64]),
     "paraiso_hydro_launch_count": (_int, [_vp, _pi64]),
     "paraiso_hydro_kernel_time": (_int, [_vp, _int, _pdbl, _pi64]),
-    "paraiso_hydro_debug_arith": (_int, [_int, _i64, _vp, _vp, _vp, _vp]),
-    "paraiso_hydro_debug_issue_cost": (_int, [_int, _dbl, _pdbl, _pdbl]),
     "paraiso_hydro_last_error": (ctypes.c_char_p, [_vp]),
     "paraiso_hydro_version": (ctypes.c_char_p, []),
 }
 
+# the probe library (include/paraiso_hydro_probe.h): tests and bench.py's roofline leg only
+PROBE_PATH = os.path.join(HERE, "libparaiso_hydro_probe.so")
+PROBE_SIGNATURES = {
+    "paraiso_probe_arith": (_int, [_int, _i64, _vp, _vp, _vp, _vp]),
+    "paraiso_probe_issue_cost": (_int, [_int, _dbl, _pdbl, _pdbl]),
+    "paraiso_probe_peak": (_int, [_int, _pdbl]),
+}
+
 _LIB = None
+_PROBE = None
 
 
 class ParaisoError(RuntimeError):
@@ -95,35 +102,58 @@ def _pointer(a):
 
 
 ISSUE_KINDS = {"ffma": 0, "fmnmx": 1, "fsetp_fsel": 2, "iadd3_lop3": 3, "ffma2": 4, "dfma": 5, "mufu": 6}
+PEAK_KINDS = {"ffma": 0, "ffma2": 1, "dfma": 2}
 
 
-def debug_issue_cost(kind, sm_clock_mhz):
-    """paraiso_hydro_debug_issue_cost: (scheduler cycles one more instruction of `kind` costs next to 16 FFMA per
+def load_probe():
+    """dlopen libparaiso_hydro_probe.so (include/paraiso_hydro_probe.h): test / measurement probes, not product."""
+    global _PROBE
+    if _PROBE is None:
+        if not os.path.exists(PROBE_PATH):
+            raise ParaisoError(PARAISO_ECUDA, f"{PROBE_PATH} not built; run `python -m paper_1204_4779_b200.build`")
+        lib = ctypes.CDLL(PROBE_PATH)
+        for name, (res, args) in PROBE_SIGNATURES.items():
+            fn = getattr(lib, name)
+            fn.restype = res
+            fn.argtypes = args
+        _PROBE = lib
+    return _PROBE
+
+
+def probe_issue_cost(kind, sm_clock_mhz):
+    """paraiso_probe_issue_cost: (scheduler cycles one more instruction of `kind` costs next to 16 FFMA per
     iteration, cycles of the 16-FFMA loop alone)."""
-    lib = load_library()
     c, base = _dbl(0.0), _dbl(0.0)
-    rc = lib.paraiso_hydro_debug_issue_cost(ISSUE_KINDS[kind] if isinstance(kind, str) else int(kind), float(sm_clock_mhz),
-                                            ctypes.byref(c), ctypes.byref(base))
+    rc = load_probe().paraiso_probe_issue_cost(ISSUE_KINDS[kind] if isinstance(kind, str) else int(kind),
+                                               float(sm_clock_mhz), ctypes.byref(c), ctypes.byref(base))
     if rc:
-        raise ParaisoError(rc, "debug_issue_cost failed")
+        raise ParaisoError(rc, "probe_issue_cost failed")
     return c.value, base.value
 
 
-def debug_arith(a, b):
-    """paraiso_hydro_debug_arith on two equal-length device tensors: returns (a / b, sqrt(|a|)) as evaluated by
-    the hot path's div_rn / sqrt_rn (device tensors of the same dtype)."""
+def probe_peak(kind):
+    """paraiso_probe_peak: measured fused multiply-adds per second / 1e12 of `kind` ("ffma", "ffma2", "dfma")."""
+    v = _dbl(0.0)
+    rc = load_probe().paraiso_probe_peak(PEAK_KINDS[kind] if isinstance(kind, str) else int(kind), ctypes.byref(v))
+    if rc:
+        raise ParaisoError(rc, "probe_peak failed")
+    return v.value
+
+
+def probe_arith(a, b):
+    """paraiso_probe_arith on two equal-length device tensors: returns (a / b, sqrt(|a|)) as evaluated by the hot
+    path's div_rn / sqrt_rn (device tensors of the same dtype)."""
     import torch
 
-    lib = load_library()
     pa, dt, n = _pointer(a)
     pb, dtb, nb = _pointer(b)
     if dt != dtb or n != nb or not a.is_cuda or not b.is_cuda:
-        raise ValueError("debug_arith wants two device tensors of equal dtype and length")
+        raise ValueError("probe_arith wants two device tensors of equal dtype and length")
     q, r = torch.empty_like(a), torch.empty_like(a)
     torch.cuda.synchronize()
-    rc = lib.paraiso_hydro_debug_arith(0 if dt == np.dtype(np.float32) else 1, n, pa, pb, q.data_ptr(), r.data_ptr())
-    if rc != PARAISO_OK:
-        raise ParaisoError(rc, lib.paraiso_hydro_last_error(None).decode())
+    rc = load_probe().paraiso_probe_arith(0 if dt == np.dtype(np.float32) else 1, n, pa, pb, q.data_ptr(), r.data_ptr())
+    if rc:
+        raise ParaisoError(rc, "probe_arith failed")
     return q, r
 
 

@@ -215,14 +215,7 @@ __device__ __forceinline__ void tma_row(void* dst, const void* src, int bytes, u
                : "memory");
 }
 
-#ifdef PH_EXPERIMENT_NO_BARRIER  // timing ablation of profiles/r1c_README.md (racy, wrong results); never defined by build.py
-__device__ __forceinline__ void block_barrier() { __syncwarp(); }
-#else
 __device__ __forceinline__ void block_barrier() { asm volatile("bar.sync 0;" ::: "memory"); }
-#endif
-#ifdef PH_PACK_NOBAR
-#define block_barrier __syncwarp
-#endif
 
 template <class T, int D, int RS, int STAGE, int NWX, int TY, int MINB, bool TMA, int RPT>
 __global__ void __launch_bounds__(MarchShape<T, D, NWX, TY, TMA, RPT>::NT, MINB)
@@ -478,7 +471,7 @@ __global__ void __launch_bounds__(MarchShape<T, D, NWX, TY, TMA, RPT>::NT, MINB)
     }
   } else {
     // =========================================================================== the halo warp
-    // It loads the x halo cells of every plane (the y halo rows are filled by four of the main warps) and
+    // It loads the whole 2-cell star halo of every plane (x halo cells and y halo rows), converts it to primitives and
     // computes the faces the tile cannot get from its own cells.  Its face tasks read only the shared plane and
     // the low-side states the main warps publish, so it never waits for anything but the block barriers.
     constexpr int NXP = (Sh::XHALO_LANES + 31) / 32;  // x halo slots per lane
@@ -742,11 +735,6 @@ bool launch_march_stage(const Real* Uin, const Real* Ubase, Real* Uout, const Ge
       if (tma && ty == 7) return launch_march_shape<Real, D, RS, STAGE, 1, 7, minb, true>(Uin, Ubase, Uout, g, sc, stream, depth);
       if (block[2] == 2 && ty == 7 && !packed)  // two rows per thread: a 32 x 14 tile, one 256-thread block per SM
         return launch_march_shape<Real, D, RS, STAGE, 1, 7, PH_RPT2_MINB, false, 2>(Uin, Ubase, Uout, g, sc, stream, depth);
-      if constexpr (can_pack) {  // EXPERIMENT r2: packed shapes under tighter register caps
-        if (packed && block[2] == 3 && ty == 5) return launch_march_shape<f32x2, D, RS, STAGE, 1, 5, 2>(Uin, Ubase, Uout, g, sc, stream, depth);
-        if (packed && block[2] == 3 && ty == 7) return launch_march_shape<f32x2, D, RS, STAGE, 1, 7, 2>(Uin, Ubase, Uout, g, sc, stream, depth);
-        if (packed && ty == 11) return launch_march_shape<f32x2, D, RS, STAGE, 1, 11, 1>(Uin, Ubase, Uout, g, sc, stream, depth);
-      }
       PH_SHAPE(4) PH_SHAPE(7) PH_SHAPE(8) PH_SHAPE(15)
 #undef PH_SHAPE
       return false;

@@ -173,7 +173,7 @@ __global__ void __launch_bounds__(PackShape<D, NWX, TY>::NT, MINB)
       // marching axis: V[m+2] (its U_in was copied during the previous iteration), slope of cell m+1, flux through
       // face m+1/2; then the copies of U_in of plane m+3 (next iteration) and of the own-cell U_base of plane m (phase C)
       T dFm[NF];
-      {
+      auto z_part = [&]() {
         cp_async_wait_all();
         T un[NF];
 #pragma unroll
@@ -198,9 +198,11 @@ __global__ void __launch_bounds__(PackShape<D, NWX, TY>::NT, MINB)
           dFm[f] = lds<T>(&sm.Fp[f][row][c0]) - Fn[f];
           sts(&sm.Fp[f][row][c0], Fn[f]);
         }
-      }
+      };
       // x slopes; the low-side state goes to the left neighbour at once (shuffle), lane 31 is patched after the barrier
       T hix[NF], rs[NF];
+      T hiy[(D == 3) ? NF : 1];
+      auto xy_slopes = [&]() {
 #pragma unroll
       for (int f = 0; f < NF; ++f) {
         const T l = xshift_left(vc[f], sm.V[s0][f][pr][pc - 1]);
@@ -211,7 +213,6 @@ __global__ void __launch_bounds__(PackShape<D, NWX, TY>::NT, MINB)
         if (lane == 0) sm.LOx[f][row][wx] = lox.v.x;
         rs[f] = xshift_right(lox, shfl_dn(lox.v.x));
       }
-      T hiy[(D == 3) ? NF : 1];
       if constexpr (D == 3) {
 #pragma unroll
         for (int f = 0; f < NF; ++f) {
@@ -220,6 +221,9 @@ __global__ void __launch_bounds__(PackShape<D, NWX, TY>::NT, MINB)
           hiy[f] = rfma(0.5f, dy, vc[f]);
         }
       }
+      };
+      z_part();
+      xy_slopes();
       block_barrier();
 
       // ------------------------------------------------------------ phase B: one Riemann solve per in-plane face

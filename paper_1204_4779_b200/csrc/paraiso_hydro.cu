@@ -45,6 +45,8 @@ PH_EXTERN_PACK(3, RIEMANN_HLLC, 1) PH_EXTERN_PACK(3, RIEMANN_HLLC, 2) PH_EXTERN_
 
 enum { VARIANT_FUSED = 0, VARIANT_MANIFEST_FLUX = 1, VARIANT_MANIFEST_ALL = 2, VARIANT_DELAYED = 3, VARIANT_MARCH = 4,
        VARIANT_FUSED1 = 5, VARIANT_PACK = 6 };
+enum { KERNEL_NONE = 0, KERNEL_MANIFEST_FLUX = 1, KERNEL_MANIFEST_ALL = 2, KERNEL_DELAYED = 3, KERNEL_MARCH = 4,
+       KERNEL_FUSED1 = 5, KERNEL_PACK = 6 };
 
 struct paraiso_hydro {
   int dims = 0, dtype = 0, nf = 0;
@@ -72,6 +74,8 @@ struct paraiso_hydro {
   cudaStream_t stream = nullptr;
   bool has_state = false;
   int64_t launches = 0;
+  int kernel_used = 0;       // KERNEL_*: the stage kernel of the last launch (get_option "kernel_used")
+  bool shape_error = false;  // a requested kernel / launch shape did not cover the grid
 
   // optional per-stage CUDA-event timing on the handle's stream (paraiso_hydro_kernel_time)
   bool timing = false;
@@ -81,7 +85,6 @@ struct paraiso_hydro {
   int64_t timed_count = 0;
 
   cudaGraphExec_t graph_exec = nullptr;
-  int graph_key = -1;  // option fingerprint the graph was captured with
   int graph_steps = 0;
 
   std::string err;
@@ -166,7 +169,6 @@ static cudaEvent_t next_event(paraiso_hydro* h) {
 static void drop_graph(paraiso_hydro* h) {
   if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
   h->graph_exec = nullptr;
-  h->graph_key = -1;
 }
 
 // Manifest intermediates are allocated on first use of a Manifest variant.
@@ -248,6 +250,7 @@ struct Launch {
         if constexpr (D > 1) recon_riemann<1>(h, g);
         if constexpr (D > 2) recon_riemann<2>(h, g);
         update<STAGE>(h, g, Uout);
+        h->kernel_used = KERNEL_MANIFEST_ALL;
         break;
       }
       case VARIANT_MANIFEST_FLUX: {
@@ -255,40 +258,83 @@ struct Launch {
         if constexpr (D > 1) flux<1>(h, g, Uin);
         if constexpr (D > 2) flux<2>(h, g, Uin);
         update<STAGE>(h, g, Uout);
+        h->kernel_used = KERNEL_MANIFEST_FLUX;
         break;
       }
-      case VARIANT_PACK:
-        if constexpr (sizeof(Real) == 4 && D >= 2) {
-          if (launch_pack_stage<D, RS, STAGE>((const float*)Uin, (const float*)stage_base<STAGE>(h), (float*)Uout, g, h->sc,
-                                              h->stream, h->block, h->tile_depth)) {
-            h->launches += 1;
-            break;
-          }
+      default:
+        on_chip_stage<STAGE>(h, g, Uin, Uout);
+    }
+  }
+
+  // The on-chip end of the Manifest <-> Delayed axis: one kernel per stage.  Which kernel runs is recorded in
+  // h->kernel_used (get_option "kernel_used").  An explicitly requested kernel (variant = pack / march / fused1 /
+  // delayed), or the default one with any launch-shape option set, that does not cover the grid or the shape is an
+  // error (PARAISO_EINVAL from the calling entry point), not a silent fallback; only variant = fused with all-default
+  // options walks down the list pack -> march -> fused1 -> delayed.
+  template <int STAGE>
+  static void on_chip_stage(paraiso_hydro* h, const Geom<Real>& g, const Real* Uin, Real* Uout) {
+    const Real* base = stage_base<STAGE>(h);
+    auto try_pack = [&]() -> bool {
+      if constexpr (sizeof(Real) == 4 && D >= 2) {
+        if (h->cells_per_thread == 0 && h->staging == 0 && h->arith == 0 &&
+            launch_pack_stage<D, RS, STAGE>((const float*)Uin, (const float*)base, (float*)Uout, g, h->sc, h->stream,
+                                            h->block, h->tile_depth)) {
+          h->kernel_used = KERNEL_PACK;
+          return true;
         }
-        // shapes the packed kernel does not cover (fp64, 1-D, odd n_x): the default on-chip kernel
-      case VARIANT_FUSED:  // the faster of the two on-chip designs per grid kind (profiles/r1d_tune_*.txt):
-                           // k_march in 3-D and in 2-D fp32, k_fused in 2-D fp64
-      case VARIANT_MARCH:
-        if ((h->variant == VARIANT_MARCH || D == 3 || sizeof(Real) == 4) &&
-            launch_march_stage<Real, D, RS, STAGE>(Uin, stage_base<STAGE>(h), Uout, g, h->sc, h->stream, h->block,
-                                                   h->tile_depth, h->cells_per_thread, h->staging, h->arith)) {
-          h->launches += 1;
-          break;
+      }
+      return false;
+    };
+    auto try_march = [&]() -> bool {
+      if (launch_march_stage<Real, D, RS, STAGE>(Uin, base, Uout, g, h->sc, h->stream, h->block, h->tile_depth,
+                                                 h->cells_per_thread, h->staging, h->arith)) {
+        h->kernel_used = KERNEL_MARCH;
+        return true;
+      }
+      return false;
+    };
+    auto try_fused1 = [&]() -> bool {
+      if (h->cells_per_thread == 0 && h->staging == 0 && h->arith == 0 &&
+          launch_fused_stage<Real, D, RS, STAGE>(Uin, base, Uout, g, h->sc, h->stream, h->block, h->tile_depth)) {
+        h->kernel_used = KERNEL_FUSED1;
+        return true;
+      }
+      return false;
+    };
+    auto try_delayed = [&]() -> bool {
+      const int bs = h->block[0] > 0 ? h->block[0] : 128;
+      if (bs > 128 || h->block[1] || h->block[2] || h->tile_depth || h->cells_per_thread || h->staging || h->arith) return false;
+      k_delayed<Real, D, RS, STAGE><<<grid1d(h->N, bs), bs, 0, h->stream>>>(Uin, base, Uout, g, h->sc);
+      h->kernel_used = KERNEL_DELAYED;
+      return true;
+    };
+    const bool shaped = h->block[0] || h->block[1] || h->block[2] || h->tile_depth || h->cells_per_thread || h->staging || h->arith;
+    bool ok = false;
+    switch (h->variant) {
+      case VARIANT_PACK: ok = try_pack(); break;
+      case VARIANT_MARCH: ok = try_march(); break;
+      case VARIANT_FUSED1: ok = try_fused1(); break;
+      case VARIANT_DELAYED: ok = try_delayed(); break;
+      default: {  // VARIANT_FUSED: the fastest on-chip kernel per grid kind (profiles/r2_tune_*.txt)
+        if (D == 1) {
+          ok = try_delayed();
+        } else if (sizeof(Real) == 4) {
+          // fp32: the packed kernel (even n_x); the options only k_march knows (cells_per_thread, staging, arith)
+          // select k_march
+          const bool march_only = h->cells_per_thread || h->staging || h->arith;
+          ok = march_only ? try_march() : (try_pack() || try_march());
+        } else if (D == 2) {
+          ok = try_fused1();
+        } else {
+          ok = try_march();
         }
-        // shapes the marching kernel does not cover: the first fused design
-      case VARIANT_FUSED1:
-        if (launch_fused_stage<Real, D, RS, STAGE>(Uin, stage_base<STAGE>(h), Uout, g, h->sc, h->stream, h->block,
-                                                   h->tile_depth)) {
-          h->launches += 1;
-          break;
-        }
-        // 1-D grids (and shapes the marching kernel does not cover) use the Delayed kernel: fall through
-      default: {
-        const int bs = h->block[0] > 0 ? h->block[0] : 128;
-        k_delayed<Real, D, RS, STAGE><<<grid1d(h->N, bs), bs, 0, h->stream>>>(Uin, stage_base<STAGE>(h), Uout, g, h->sc);
-        h->launches += 1;
+        if (!ok && !shaped) ok = try_march() || try_fused1() || try_delayed();
       }
     }
+    if (ok)
+      h->launches += 1;
+    else
+      h->shape_error = true;
   }
 
   static void step(paraiso_hydro* h) {
@@ -337,31 +383,15 @@ static void dispatch(paraiso_hydro* h, F&& f) {
 #undef PH_CASE
 }
 
-// the hot path's division and square root (hydro_math.cuh div_rn / sqrt_rn), exposed for tests
-template <class Real>
-__global__ void k_debug_arith(long long n, const Real* a, const Real* b, Real* quot, Real* root) {
-  const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-  if (i >= n) return;
-  quot[i] = div_rn(a[i], b[i]);
-  root[i] = sqrt_rn(rabs(a[i]));
-}
-
 static int check_launch(paraiso_hydro* h) {
+  if (h->shape_error) {
+    h->shape_error = false;
+    cudaGetLastError();
+    return fail(h, PARAISO_EINVAL, "the requested kernel variant / launch shape does not cover this grid (shape not covered)");
+  }
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail(h, PARAISO_ECUDA, std::string("kernel launch: ") + cudaGetErrorString(e));
   return PARAISO_OK;
-}
-
-static int options_key(const paraiso_hydro* h) {
-  int k = h->boundary | (h->riemann << 1) | (h->integrator << 2) | (h->variant << 3);
-  k = k * 1031 + h->block[0];
-  k = k * 1031 + h->block[1];
-  k = k * 1031 + h->block[2];
-  k = k * 1031 + h->tile_depth;
-  k = k * 1031 + h->cells_per_thread;
-  k = k * 7 + h->staging;
-  k = k * 3 + h->arith;
-  return k & 0x7fffffff;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -452,7 +482,8 @@ static bool find_option(paraiso_hydro* h, const char* key, OptionRef* ref) {
                       {"state_kind", {&h->state_kind, 0, 1}},
                       {"integrator", {&h->integrator, 0, 1}},
                       {"staging", {&h->staging, 0, 2}},
-                      {"arith", {&h->arith, 0, 1}}};
+                      {"arith", {&h->arith, 0, 1}},
+                      {"kernel_used", {&h->kernel_used, 0, 0}}};  // read-only: KERNEL_* of the last stage launch
   for (const Opt& o : opts)
     if (!std::strcmp(key, o.key)) {
       *ref = o.ref;
@@ -466,6 +497,7 @@ int paraiso_hydro_set_option(paraiso_hydro_t* h, const char* key, int64_t value)
   OptionRef r;
   if (!find_option(h, key, &r)) return fail(h, PARAISO_EINVAL, std::string("set_option: unknown key ") + key);
   if (value < r.lo || value > r.hi) return fail(h, PARAISO_EINVAL, std::string("set_option: value out of range for ") + key);
+  if (*r.field != int(value)) drop_graph(h);  // a captured graph is valid only for the options it was captured with
   *r.field = int(value);
   return PARAISO_OK;
 }
@@ -562,6 +594,11 @@ static int capture_graph(paraiso_hydro* h, int nsteps) {
   }
   h->launches = before;
   h->stream = user;
+  if (h->shape_error) {
+    if (graph) cudaGraphDestroy(graph);
+    cudaStreamDestroy(cap);
+    return check_launch(h);
+  }
   if (e == cudaSuccess) e = cudaGraphInstantiate(&h->graph_exec, graph, 0);
   if (graph) cudaGraphDestroy(graph);
   cudaStreamDestroy(cap);
@@ -569,7 +606,6 @@ static int capture_graph(paraiso_hydro* h, int nsteps) {
     h->graph_exec = nullptr;
     return fail(h, PARAISO_ECUDA, std::string("graph capture: ") + cudaGetErrorString(e));
   }
-  h->graph_key = options_key(h);
   h->graph_steps = nsteps;
   return PARAISO_OK;
 }
@@ -586,7 +622,7 @@ static int enqueue_steps(paraiso_hydro* h, int64_t nsteps) {
   const int chunk = 8;  // steps per graph
   int64_t left = nsteps;
   if (h->use_graph && !h->timing && nsteps >= chunk) {
-    if (!h->graph_exec || h->graph_key != options_key(h) || h->graph_steps != chunk) {
+    if (!h->graph_exec || h->graph_steps != chunk) {
       int rc = capture_graph(h, chunk);
       if (rc) return rc;
     }
@@ -626,7 +662,9 @@ int paraiso_hydro_run(paraiso_hydro_t* h, double cfl, int64_t nsteps, double t_e
   } st = {0, 0, 0};
   long long steps0 = 0;
   CUDA_TRY(h, cudaMemcpyAsync(&steps0, &h->sc->steps, sizeof(long long), cudaMemcpyDeviceToHost, h->stream));
+  CUDA_TRY(h, cudaMemcpyAsync(&st.t, &h->sc->t, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
   CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+  st.steps = steps0;  // nsteps == 0: nothing runs, report the current clock
   int64_t issued = 0;
   while (issued < nsteps) {
     const int64_t c = std::min<int64_t>(64, nsteps - issued);
@@ -691,21 +729,6 @@ int paraiso_hydro_kernel_time(paraiso_hydro_t* h, int enable, double* total_ms, 
   }
   if (total_ms) *total_ms = h->timed_ms;
   if (stage_launches) *stage_launches = h->timed_count;
-  return PARAISO_OK;
-}
-
-int paraiso_hydro_debug_arith(int dtype, int64_t n, const void* a, const void* b, void* quot, void* root) {
-  if (n < 0 || !a || !b || !quot || !root) return fail(nullptr, PARAISO_EINVAL, "debug_arith: bad argument");
-  if (dtype != PARAISO_F32 && dtype != PARAISO_F64) return fail(nullptr, PARAISO_EINVAL, "debug_arith: bad dtype");
-  if (n == 0) return PARAISO_OK;
-  const unsigned int blocks = (unsigned int)((n + 255) / 256);
-  if (dtype == PARAISO_F32)
-    k_debug_arith<float><<<blocks, 256>>>((long long)n, (const float*)a, (const float*)b, (float*)quot, (float*)root);
-  else
-    k_debug_arith<double><<<blocks, 256>>>((long long)n, (const double*)a, (const double*)b, (double*)quot, (double*)root);
-  cudaError_t e = cudaGetLastError();
-  if (e == cudaSuccess) e = cudaDeviceSynchronize();
-  if (e != cudaSuccess) return fail(nullptr, PARAISO_ECUDA, std::string("debug_arith: ") + cudaGetErrorString(e));
   return PARAISO_OK;
 }
 

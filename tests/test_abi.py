@@ -39,6 +39,22 @@ def test_library_exports_every_declared_symbol(lib):
     assert set(binding.SIGNATURES) == set(names)
 
 
+def test_probe_library_exports_every_declared_symbol(lib):
+    """include/paraiso_hydro_probe.h: the test / measurement probes live in a library of their own."""
+    from paper_1204_4779_b200 import binding
+
+    text = re.sub(r"/\*.*?\*/", "", open(os.path.join(ROOT, "include", "paraiso_hydro_probe.h")).read(), flags=re.S)
+    names = sorted(set(re.findall(r"\b(paraiso_probe_[a-z_]+)\s*\(", text)))
+    assert names == sorted(binding.PROBE_SIGNATURES)
+    raw = ctypes.CDLL(binding.PROBE_PATH)
+    for name in names:
+        assert hasattr(raw, name), name
+    product = ctypes.CDLL(binding.LIB_PATH)
+    for name in names:
+        assert not hasattr(product, name), "probes must not be exported by the product library"
+    assert not hasattr(product, "paraiso_hydro_debug_arith")
+
+
 def test_version_and_error_strings_need_no_device(lib):
     assert lib.paraiso_hydro_version().decode().startswith("paraiso_hydro")
     assert isinstance(lib.paraiso_hydro_last_error(None), bytes)

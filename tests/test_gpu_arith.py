@@ -34,7 +34,7 @@ def test_div_and_sqrt_are_correctly_rounded_in_the_normal_range(dtype):
         a[1000:2000] = np.nextafter(b[1000:2000], dtype(np.inf))
         a[2000:3000] = 0.0
         b[3000:4000] = np.ldexp(1.0, np.arange(1000) % 41 - 20).astype(dtype)
-        q, r = binding.debug_arith(torch.from_numpy(a).cuda(), torch.from_numpy(b).cuda())
+        q, r = binding.probe_arith(torch.from_numpy(a).cuda(), torch.from_numpy(b).cuda())
         q, r = q.cpu().numpy(), r.cpu().numpy()
         with np.errstate(all="ignore"):
             qref, rref = a / b, np.sqrt(np.abs(a))
@@ -57,8 +57,8 @@ def test_issue_cost_of_the_instruction_classes():
                                    capture_output=True, text=True, timeout=30).stdout.split()[0])
     except Exception:
         mhz = 1965.0
-    cost = {k: binding.debug_issue_cost(k, mhz)[0] for k in binding.ISSUE_KINDS}
-    base = binding.debug_issue_cost("ffma", mhz)[1]
+    cost = {k: binding.probe_issue_cost(k, mhz)[0] for k in binding.ISSUE_KINDS}
+    base = binding.probe_issue_cost("ffma", mhz)[1]
     print("issue cost in scheduler cycles per instruction:", {k: round(v, 2) for k, v in cost.items()}, "16-FFMA loop:", round(base, 1))
     assert 16.0 <= base <= 30.0            # 16 FFMA + loop control at about one instruction per cycle
     assert 0.8 <= cost["ffma"] <= 1.4
@@ -66,3 +66,16 @@ def test_issue_cost_of_the_instruction_classes():
         assert 1.4 <= cost[k] <= 2.6, (k, cost[k])
     assert 1.6 <= cost["ffma2"] <= 2.6 and 1.6 <= cost["dfma"] <= 2.6
     assert cost["mufu"] >= 1.6
+
+
+def test_measured_peak_lane_rates():
+    """paraiso_probe_peak: the measured denominators of roofline (b).  FFMA2 reaches the nominal FP32 lane rate
+    (148 SMs x 128 lanes x clock), scalar FFMA stays below it, DFMA is half the FP32 rate."""
+    from paper_1204_4779_b200 import binding
+
+    pk = {k: binding.probe_peak(k) for k in binding.PEAK_KINDS}
+    print("measured peak, Tera fused-multiply-adds/s:", {k: round(v, 2) for k, v in pk.items()})
+    nominal = 148 * 128 * 1.965e9 / 1e12
+    assert 0.5 * nominal <= pk["ffma"] <= 1.05 * nominal
+    assert 0.7 * nominal <= pk["ffma2"] <= 1.05 * nominal
+    assert 0.25 * nominal <= pk["dfma"] <= 0.55 * nominal

@@ -4,7 +4,11 @@
   configs 1, 2, 3  the oracle (OpenMP build, bit-identical to the serial one) runs the whole config; every cell is
                    compared after the full number of steps with north_star's 100-step tolerance (R17
                    metric) and after one step with the one-step tolerance; t and the step count must agree.
-  config 4         512^3 x 20 steps is ~3 x 10^9 oracle cell-steps: instead (a) dt of the first step against the
+  config 4         test_config4_full_grid_full_length: the OpenMP oracle runs all 20 steps of the 512^3 grid (~3 x 10^9
+                   cell-steps, a few minutes on the box's host cores, ~14 GB of host memory); EVERY cell is compared
+                   after step 1 (default variant and each end of the Manifest <-> Delayed axis: manifest_all,
+                   manifest_flux, delayed, march, pack) and after step 20 (default variant).  The older sampled test is
+                   kept as a fast pre-check: (a) dt of the first step against the
                    oracle's CFL reduction over the full state, (b) the first step on SAMPLED sub-boxes: one RK2 step
                    reaches 4 cells, so the oracle advances a sub-box cut (with periodic wrap) from the full initial
                    state with a 6-cell margin and its interior is compared cell by cell with the GPU's full-grid
@@ -16,7 +20,7 @@ Inputs never come from the CUDA path: the oracle always starts from the seeded i
 import numpy as np
 import pytest
 
-from parity_util import TOL, field_errors
+from parity_util import TOL, field_errors, own_scale_errors
 from paper_1204_4779_b200 import inputs
 
 pytestmark = [pytest.mark.gpu, pytest.mark.slow]
@@ -149,3 +153,50 @@ def test_config4_first_step_on_sampled_boxes_and_properties(gpu, oracle_mod):
     assert abs(sums[4] - sums0[4]) <= 2e-6 * abs(sums0[4])                 # energy
     mom_scale = np.abs(G[1:4]).max() * cells
     assert np.all(np.abs(sums[1:4] - sums0[1:4]) <= 2e-6 * mom_scale)      # momentum (zero in total at t = 0)
+
+
+def test_config4_full_grid_full_length(gpu, oracle_mod):
+    """BASELINE config 4 at full size AND full length, every cell (north_star: "on all five configs"; SURVEY §8(c3):
+    configs with fewer than 100 steps are checked after 1 step and after their full length).  512^3 is the only config
+    whose 32-bit element offsets come near their limit (nf N = 6.7e8)."""
+    import torch
+
+    w = inputs.baseline_config(4)
+    tol1, tol100, toldt = TOL[np.dtype(w.dtype)]
+    (ref1, rdt1), ref, rt = oracle_run(oracle_mod, w, w.steps)
+
+    def first_step(variant):
+        with gpu.ParaisoHydro(w.n, w.extent, w.gamma, w.dtype, w.boundary, "hllc", variant) as h:
+            h.set_state(torch.from_numpy(w.U).cuda())
+            gdt = h.cfl_dt(w.cfl)
+            assert abs(gdt - rdt1) <= toldt * rdt1, (variant, gdt, rdt1)
+            h.run(w.cfl, 1)
+            got1 = h.get_state()
+            assert h.stats() == 0
+        err = field_errors(got1, ref1)
+        assert np.all(err <= tol1), (variant, err)
+        assert np.array_equal(got1, ref1), (variant, "same written arithmetic as the oracle: bit-equal")
+        return err
+
+    # both ends of the Manifest <-> Delayed axis and both on-chip designs, first step, every cell
+    for variant in ("manifest_all", "manifest_flux", "delayed", "march", "pack"):
+        first_step(variant)
+
+    # the default variant (what bench.py times): step 1 and the full 20 steps, device-paced run with graph replay
+    with gpu.ParaisoHydro(w.n, w.extent, w.gamma, w.dtype, w.boundary, "hllc") as h:
+        h.set_state(torch.from_numpy(w.U).cuda())
+        h.run(w.cfl, 1)
+        got1 = h.get_state()
+        assert np.all(field_errors(got1, ref1) <= tol1)
+        assert np.array_equal(got1, ref1)
+        del got1
+        h.run(w.cfl, w.steps - 1)
+        got = h.get_state()
+        t, k = h.time()
+        assert h.stats() == 0 and k == w.steps
+    assert abs(t - rt) <= 10 * toldt * rt, (t, rt)
+    err = field_errors(got, ref)
+    assert np.all(err <= tol100), err
+    assert np.all(own_scale_errors(got, ref) <= tol100)
+    print(f"config 4: {w.steps} steps on 512^3, max field error {err.max():.2e}, bit-equal {np.array_equal(got, ref)}")
+    assert np.array_equal(got, ref)
