@@ -20,7 +20,7 @@
 
 namespace ph {
 
-template <int D, int NWX, int TY>
+template <int D, int NWX, int TY, int NH = 1>
 struct PackShape {
   using T = f32x2;
   static constexpr int NF = D + 2;
@@ -29,9 +29,10 @@ struct PackShape {
   static constexpr int PY = (D == 3) ? TY + 4 : 1;
   static constexpr int OY = (D == 3) ? 2 : 0;
   static constexpr int NMAIN = NWX * TY * 32;
-  static constexpr int NT = NMAIN + 32;
+  static constexpr int NT = NMAIN + 32 * NH;               // NH halo warps follow the main warps
   static constexpr int XROWS = (D == 3) ? TY : 1;
   static_assert(D == 2 || D == 3, "2-D and 3-D grids");
+  static_assert(NH == 1 || (NH == 2 && D == 3), "two halo warps (one for the y faces, one for the x faces): 3-D only");
   static_assert(D == 3 || TY == 1, "2-D tiles are rows");
   static_assert(D == 2 || NWX == 1, "3-D tiles are one warp wide");
   static_assert(XROWS <= 64, "tile too tall for one halo warp");
@@ -60,10 +61,10 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 
 // BND: the boundary mode as a compile-time constant.  On periodic grids (n_x even) every pair of cells a thread
 // touches, ghost pairs included, is one aligned 8-byte pair in memory; outflow ghosts are clamped cell by cell.
-template <int D, int RS, int STAGE, int NWX, int TY, int MINB, int BND>
-__global__ void __launch_bounds__(PackShape<D, NWX, TY>::NT, MINB)
+template <int D, int RS, int STAGE, int NWX, int TY, int MINB, int BND, int NH>
+__global__ void __launch_bounds__(PackShape<D, NWX, TY, NH>::NT, MINB)
     k_pack(const float* __restrict__ Uin, const float* Ubase, float* Uout, Geom<float> g, Scalars* sc, int depth) {
-  using Sh = PackShape<D, NWX, TY>;
+  using Sh = PackShape<D, NWX, TY, NH>;
   using T = f32x2;
   using P = Prim<T, D>;
   constexpr int NF = Sh::NF, TXC = Sh::TXC, OY = Sh::OY, XROWS = Sh::XROWS;
@@ -292,7 +293,12 @@ __global__ void __launch_bounds__(PackShape<D, NWX, TY>::NT, MINB)
   } else {
     // =========================================================================== the halo warp
     // Loads the 2-cell star halo of every plane, converts it to primitives (into the ring slot of the NEXT plane) and
-    // computes the faces the tile cannot get from its own cells.
+    // computes the faces the tile cannot get from its own cells.  NH = 2: the first halo warp serves the y direction
+    // (halo rows, the faces below / above the tile), the second the x direction, so that neither has more work per
+    // plane than a main warp and the block barriers do not wait for them.
+    const int hw = warp - NWX * TY;
+    const bool do_y = (D == 3) && (NH == 1 || hw == 0);
+    const bool do_x = (NH == 1 || hw == NH - 1);
     constexpr int XHALO = 2 * XROWS;                    // x halo pairs per plane: rows x {left pair, right pair}
     constexpr int NXP = (XHALO + 31) / 32;
     CellSrc hsrc[NXP];
@@ -301,7 +307,7 @@ __global__ void __launch_bounds__(PackShape<D, NWX, TY>::NT, MINB)
 #pragma unroll
     for (int q = 0; q < NXP; ++q) {
       const int id = lane + 32 * q;
-      hval[q] = id < XHALO;
+      hval[q] = do_x && id < XHALO;
       const int r = hval[q] ? (id >> 1) : 0;
       const int px = (id & 1) ? TXC + 2 : 0;
       hpy[q] = r + OY;
@@ -321,10 +327,12 @@ __global__ void __launch_bounds__(PackShape<D, NWX, TY>::NT, MINB)
 #pragma unroll
           for (int f = 0; f < NF; ++f) Uh[q][f] = ldg_pair(Uin, f * Ni + pl, hsrc[q]);
         }
+      if (do_y) {
 #pragma unroll
-      for (int q = 0; q < NYP; ++q) {
+        for (int q = 0; q < NYP; ++q) {
 #pragma unroll
-        for (int f = 0; f < NF; ++f) Uyh[q][f] = ldg_pair(Uin, f * Ni + pl, ysrc[q]);
+          for (int f = 0; f < NF; ++f) Uyh[q][f] = ldg_pair(Uin, f * Ni + pl, ysrc[q]);
+        }
       }
     };
     auto store_halo = [&](int s) {
@@ -336,16 +344,18 @@ __global__ void __launch_bounds__(PackShape<D, NWX, TY>::NT, MINB)
 #pragma unroll
           for (int f = 0; f < NF; ++f) sts(&sm.V[s][f][hpy[q]][hpx[q]], u[f]);
         }
+      if (do_y) {
 #pragma unroll
-      for (int q = 0; q < NYP; ++q) {
-        prim_to_fields<T, D>(prim_of<T, D>(Uyh[q], g.gm1), u);
+        for (int q = 0; q < NYP; ++q) {
+          prim_to_fields<T, D>(prim_of<T, D>(Uyh[q], g.gm1), u);
 #pragma unroll
-        for (int f = 0; f < NF; ++f) sts(&sm.V[s][f][q < 2 ? q : TY + q][lane * W + 2], u[f]);
+          for (int f = 0; f < NF; ++f) sts(&sm.V[s][f][q < 2 ? q : TY + q][lane * W + 2], u[f]);
+        }
       }
     };
     // x face tasks: lane l handles tile rows ra (first lane of T) and rb (second lane)
     constexpr int XTASK_LANES = (XROWS + 1) / 2;
-    const bool xtask = lane < XTASK_LANES;
+    const bool xtask = do_x && lane < XTASK_LANES;
     const int ra = xtask ? lane : 0;
     const int rb = min(ra + XTASK_LANES, XROWS - 1);
     auto plane_x = [&](int s, int qx) {
@@ -372,7 +382,7 @@ __global__ void __launch_bounds__(PackShape<D, NWX, TY>::NT, MINB)
       // ---- phase A: high-side states of the cells just below the tile, low-side states of those just above;
       //      primitives of the next plane's halo (loaded during the previous phase B)
       P hiYlow, hiXlow;
-      if constexpr (D == 3) {
+      if constexpr (D == 3) if (do_y) {
         interpolate<T, D>(plane_y(s0, 0), plane_y(s0, 1), plane_y(s0, 2), nullptr, &hiYlow);
         P lo;
         interpolate<T, D>(plane_y(s0, TY + 1), plane_y(s0, TY + 2), plane_y(s0, TY + 3), &lo, nullptr);
@@ -396,7 +406,7 @@ __global__ void __launch_bounds__(PackShape<D, NWX, TY>::NT, MINB)
       if (more) store_halo(s1);
       block_barrier();
       // ---- phase B: flux through the tile's low faces; loads of the halo of plane m+2
-      if constexpr (D == 3) {
+      if constexpr (D == 3) if (do_y) {
         T a[NF], F[NF];
 #pragma unroll
         for (int f = 0; f < NF; ++f) a[f] = lds<T>(&sm.LOy[f][0][lane * W]);
@@ -430,11 +440,11 @@ __global__ void __launch_bounds__(PackShape<D, NWX, TY>::NT, MINB)
 }
 
 // ------------------------------------------------------------------------------------------------
-template <int D, int RS, int STAGE, int NWX, int TY, int MINB, int BND>
+template <int D, int RS, int STAGE, int NWX, int TY, int MINB, int BND, int NH>
 static bool launch_pack_bnd(const float* Uin, const float* Ubase, float* Uout, const Geom<float>& g, Scalars* sc,
                             cudaStream_t stream, int depth) {
-  using Sh = PackShape<D, NWX, TY>;
-  auto kern = k_pack<D, RS, STAGE, NWX, TY, MINB, BND>;
+  using Sh = PackShape<D, NWX, TY, NH>;
+  auto kern = k_pack<D, RS, STAGE, NWX, TY, MINB, BND, NH>;
   static bool configured[64] = {};
   int dev = 0;
   if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return false;
@@ -459,16 +469,16 @@ static bool launch_pack_bnd(const float* Uin, const float* Ubase, float* Uout, c
   return true;
 }
 
-template <int D, int RS, int STAGE, int NWX, int TY, int MINB>
+template <int D, int RS, int STAGE, int NWX, int TY, int MINB, int NH = 1>
 static bool launch_pack_shape(const float* Uin, const float* Ubase, float* Uout, const Geom<float>& g, Scalars* sc,
                               cudaStream_t stream, int depth) {
   if (g.boundary == BOUNDARY_PERIODIC)
-    return launch_pack_bnd<D, RS, STAGE, NWX, TY, MINB, BOUNDARY_PERIODIC>(Uin, Ubase, Uout, g, sc, stream, depth);
-  return launch_pack_bnd<D, RS, STAGE, NWX, TY, MINB, BOUNDARY_OUTFLOW>(Uin, Ubase, Uout, g, sc, stream, depth);
+    return launch_pack_bnd<D, RS, STAGE, NWX, TY, MINB, BOUNDARY_PERIODIC, NH>(Uin, Ubase, Uout, g, sc, stream, depth);
+  return launch_pack_bnd<D, RS, STAGE, NWX, TY, MINB, BOUNDARY_OUTFLOW, NH>(Uin, Ubase, Uout, g, sc, stream, depth);
 }
 
 // Returns false when the packed kernel does not cover this shape (odd n_x, unknown block shape): the caller falls back.
-//   block[0] (2-D): main warps per block (0 = default); block[1] (3-D): main warps TY (0 = default)
+//   block[0] (2-D): main warps per block (0 = default); block[1] (3-D): main warps TY (0 = default; 14 = two halo warps)
 template <int D, int RS, int STAGE>
 bool launch_pack_stage(const float* Uin, const float* Ubase, float* Uout, const Geom<float>& g, Scalars* sc,
                        cudaStream_t stream, const int* block, int tile_depth) {
@@ -485,13 +495,21 @@ bool launch_pack_stage(const float* Uin, const float* Ubase, float* Uout, const 
       if (nwx == 7) return launch_pack_shape<D, RS, STAGE, 7, 1, 2>(Uin, Ubase, Uout, g, sc, stream, depth);
       return false;
     } else {
-      const int ty = block[1] > 0 ? block[1] : 7;
+      // default tile height: 14 rows + two halo warps (one block of 16 warps per SM: the halo work per cell halves and
+      // neither halo warp has more work per plane than a main warp) when the grid gives every SM several such blocks
+      // at the full marching depth; 7 rows + one halo warp (two blocks per SM) otherwise (profiles/r2_README.md)
+      int ty = block[1];
+      if (ty <= 0) {
+        const long long tiles14 = (long long)((g.n[0] + 63) / 64) * ((g.n[1] + 13) / 14);
+        ty = tiles14 * ((g.n[2] + 127) / 128) >= 4 * 148 ? 14 : 7;
+      }
       const long long tiles = (long long)((g.n[0] + 63) / 64) * ((g.n[1] + ty - 1) / ty);
       const int depth = tile_depth > 0 ? tile_depth : march_default_depth(tiles, g.n[2]);
       if (ty == 7) return launch_pack_shape<D, RS, STAGE, 1, 7, 2>(Uin, Ubase, Uout, g, sc, stream, depth);
       if (ty == 5) return launch_pack_shape<D, RS, STAGE, 1, 5, 2>(Uin, Ubase, Uout, g, sc, stream, depth);
       if (ty == 11) return launch_pack_shape<D, RS, STAGE, 1, 11, 1>(Uin, Ubase, Uout, g, sc, stream, depth);
       if (ty == 15) return launch_pack_shape<D, RS, STAGE, 1, 15, 1>(Uin, Ubase, Uout, g, sc, stream, depth);
+      if (ty == 14) return launch_pack_shape<D, RS, STAGE, 1, 14, 1, 2>(Uin, Ubase, Uout, g, sc, stream, depth);
       return false;
     }
   }

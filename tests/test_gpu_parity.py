@@ -267,6 +267,27 @@ def test_march_launch_shapes_match_oracle(gpu, oracle_mod, dims, opts, boundary)
         assert np.array_equal(got, ref), "the marching kernel states the same arithmetic as the oracle: bit-equal"
 
 
+# every launch shape of the packed kernel (variant pack): 2-D rows of 2 / 4 / 7 warps, 3-D tiles of 5 / 7 / 11 / 15 rows
+# with one halo warp and of 14 rows with two (one for the y faces, one for the x faces)
+PACK_SHAPES = [(2, {"block_x": 2}), (2, {"block_x": 4, "tile_depth": 5}), (2, {"block_x": 7}),
+               (3, {"block_y": 5}), (3, {"block_y": 7, "tile_depth": 3}), (3, {"block_y": 11}), (3, {"block_y": 15}),
+               (3, {"block_y": 14}), (3, {"block_y": 14, "tile_depth": 4})]
+
+
+@pytest.mark.parametrize("boundary", ["periodic", "outflow"])
+@pytest.mark.parametrize("dims,opts", PACK_SHAPES)
+def test_pack_launch_shapes_match_oracle(gpu, oracle_mod, dims, opts, boundary):
+    # even n_x, ragged against every tile edge, several tiles per axis (3-D: 3 tiles in x, up to 8 in y)
+    for shape in {2: [(300, 41)], 3: [(150, 37, 13), (64, 14, 9)]}[dims]:
+        w = inputs.random_smooth(shape, np.float32, seed=51 + dims, boundary=boundary)
+        ref, rdt = oracle_steps(oracle_mod, w, 3)
+        got, gdt = gpu_steps(gpu, w, 3, "pack", **opts)
+        tol1, _, toldt = TOL[np.dtype(np.float32)]
+        assert np.all(field_errors(got, ref) <= 3 * tol1), (opts, field_errors(got, ref))
+        assert all(abs(a - b) <= toldt * b for a, b in zip(gdt, rdt))
+        assert np.array_equal(got, ref), "the packed kernel states the same arithmetic as the oracle: bit-equal"
+
+
 KERNEL_ID = {"manifest_flux": 1, "manifest_all": 2, "delayed": 3, "march": 4, "fused1": 5, "pack": 6}
 
 
