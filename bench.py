@@ -38,7 +38,7 @@ if ROOT not in sys.path:
 
 METRIC = "Gcell-updates/s per RK2 step"
 UNIT = "Gcell/s"
-DEFAULT_STEPS = {0: 279, 1: 100, 2: 50, 3: 50, 4: 20}
+DEFAULT_STEPS = {0: 279, 1: 100, 2: 50, 3: 50, 4: 20, 11: 50, 13: 20}
 
 
 def measured_peaks():

@@ -48,6 +48,9 @@ __device__ __forceinline__ f32fast lane_pack(float a, float, f32fast*) { return 
 __device__ __forceinline__ float lane_last(float a) { return a; }
 __device__ __forceinline__ double lane_last(double a) { return a; }
 __device__ __forceinline__ float lane_last(f32x2 a) { return a.v.y; }
+__device__ __forceinline__ void lane_set_last(float& a, float x) { a = x; }
+__device__ __forceinline__ void lane_set_last(double& a, double x) { a = x; }
+__device__ __forceinline__ void lane_set_last(f32x2& a, float x) { a.v.y = x; }
 // the x-neighbour views of a thread's cells: (left neighbour, own cells but the last) / (own cells but the first, right)
 __device__ __forceinline__ float xshift_left(float, float nb) { return nb; }
 __device__ __forceinline__ double xshift_left(double, double nb) { return nb; }

@@ -16,15 +16,23 @@
 // lane to the scalar kernels and to the oracle (tests/test_gpu_parity.py).  n_x must be even (pairs are 8-byte
 // aligned and wrap as pairs); the launcher falls back to k_march otherwise.
 #pragma once
+#include <type_traits>
+
 #include "hydro_kernels_march.cuh"
+
+// fp64, 2-D rows: blocks per SM the register cap of __launch_bounds__ is set for
+#ifndef PH_PACK64_MINB2
+#define PH_PACK64_MINB2 4
+#endif
 
 namespace ph {
 
-template <int D, int NWX, int TY, int NH = 1>
+template <class T, int D, int NWX, int TY, int NH = 1>
 struct PackShape {
-  using T = f32x2;
+  using S = scalar_t<T>;
+  static constexpr int W = LaneTraits<T>::W;             // cells per thread: 2 (f32x2) or 1 (double); 8 bytes either way
   static constexpr int NF = D + 2;
-  static constexpr int TXC = NWX * 64;                   // cells per tile row
+  static constexpr int TXC = NWX * 32 * W;               // cells per tile row
   static constexpr int PX = TXC + 4;                     // plane row: tile + 2 halo cells on each side
   static constexpr int PY = (D == 3) ? TY + 4 : 1;
   static constexpr int OY = (D == 3) ? 2 : 0;
@@ -32,26 +40,33 @@ struct PackShape {
   static constexpr int NT = NMAIN + 32 * NH;               // NH halo warps follow the main warps
   static constexpr int XROWS = (D == 3) ? TY : 1;
   static_assert(D == 2 || D == 3, "2-D and 3-D grids");
-  static_assert(NH == 1 || (NH == 2 && D == 3), "two halo warps (one for the y faces, one for the x faces): 3-D only");
+  static_assert(NH == 1 || (NH == 2 && D == 3) || (NH == 0 && D == 2),
+                "two halo warps (one for the y faces, one for the x faces): 3-D only; no halo warp: 2-D only");
+  // NH = 0 (2-D rows): no halo warp.  Neighbouring tiles overlap by 4 cells instead: the first two and the last two cells
+  // of a tile row are ghosts that the block loads, converts and reconstructs like its own cells but never stores, so
+  // every face of an owned cell lies between two cells of the same block and x needs nothing but the warp shuffles and
+  // the warp-edge slots (2 ghost cells per side = the stencil reach).  TXO = owned cells per tile row.
+  static constexpr int GH = (NH == 0) ? 2 : 0;
+  static constexpr int TXO = TXC - 2 * GH;
   static_assert(D == 3 || TY == 1, "2-D tiles are rows");
   static_assert(D == 2 || NWX == 1, "3-D tiles are one warp wide");
-  static_assert(XROWS <= 64, "tile too tall for one halo warp");
+  static_assert((XROWS + W - 1) / W <= 32, "tile too tall for one halo warp");
   struct Smem {
-    float V[3][NF][PY][PX];                               // ring: primitives of planes m (with halo), m+1, m+2
-    float Hm[NF][XROWS][TXC];                             // high-side marching-axis state of plane m, own cells
-    float Fp[NF][XROWS][TXC];                             // flux through the marching-axis face m-1/2, own cells
-    float LOy[(D == 3) ? NF : 1][XROWS + 1][(D == 3) ? TXC : 2];  // [r]: low-side y state of tile row r (r = TY: halo warp)
-    float Fy[(D == 3) ? NF : 1][XROWS][(D == 3) ? TXC : 2];       // [r]: flux through the low y face of row r (r = 0: halo warp)
-    float Un[NF][XROWS][TXC];                             // cp.async staging: U_in of plane m+2, own cells
-    float Ub[NF][XROWS][TXC];                             // cp.async staging: U_base of plane m, own cells
-    float LOx[NF][XROWS][NWX + 1];                        // [e]: low-side x state of the first cell of warp column e
-    float Fx[NF][XROWS][NWX];                             // [e]: flux through the low x face of warp column e
+    S V[3][NF][PY][PX];                               // ring: primitives of planes m (with halo), m+1, m+2
+    S Hm[NF][XROWS][TXC];                             // high-side marching-axis state of plane m, own cells
+    S Fp[NF][XROWS][TXC];                             // flux through the marching-axis face m-1/2, own cells
+    S LOy[(D == 3) ? NF : 1][XROWS + 1][(D == 3) ? TXC : 2];  // [r]: low-side y state of tile row r (r = TY: halo warp)
+    S Fy[(D == 3) ? NF : 1][XROWS][(D == 3) ? TXC : 2];       // [r]: flux through the low y face of row r (r = 0: halo warp)
+    S Un[NF][XROWS][TXC];                             // cp.async staging: U_in of plane m+2, own cells
+    S Ub[NF][XROWS][TXC];                             // cp.async staging: U_base of plane m, own cells
+    S LOx[NF][XROWS][NWX + 1];                        // [e]: low-side x state of the first cell of warp column e
+    S Fx[NF][XROWS][NWX];                             // [e]: flux through the low x face of warp column e
   };
 };
 
 // 8-byte asynchronous copy global -> shared of one pair of cells (cp.async: SASS LDGSTS), read back by the issuing
 // thread after cp_async_wait_all(): no register is held while the load is in flight
-__device__ __forceinline__ void cp_async8(float* dst_smem, const float* src) {
+__device__ __forceinline__ void cp_async8(void* dst_smem, const void* src) {
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_addr(dst_smem)), "l"(src) : "memory");
 }
 __device__ __forceinline__ void cp_async4(float* dst_smem, const float* src) {
@@ -61,15 +76,16 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 
 // BND: the boundary mode as a compile-time constant.  On periodic grids (n_x even) every pair of cells a thread
 // touches, ghost pairs included, is one aligned 8-byte pair in memory; outflow ghosts are clamped cell by cell.
-template <int D, int RS, int STAGE, int NWX, int TY, int MINB, int BND, int NH>
-__global__ void __launch_bounds__(PackShape<D, NWX, TY, NH>::NT, MINB)
-    k_pack(const float* __restrict__ Uin, const float* Ubase, float* Uout, Geom<float> g, Scalars* sc, int depth) {
-  using Sh = PackShape<D, NWX, TY, NH>;
-  using T = f32x2;
+template <class T, int D, int RS, int STAGE, int NWX, int TY, int MINB, int BND, int NH>
+__global__ void __launch_bounds__(PackShape<T, D, NWX, TY, NH>::NT, MINB)
+    k_pack(const scalar_t<T>* __restrict__ Uin, const scalar_t<T>* Ubase, scalar_t<T>* Uout, Geom<scalar_t<T>> g, Scalars* sc,
+           int depth) {
+  using Sh = PackShape<T, D, NWX, TY, NH>;
+  using S = scalar_t<T>;
   using P = Prim<T, D>;
   constexpr int NF = Sh::NF, TXC = Sh::TXC, OY = Sh::OY, XROWS = Sh::XROWS;
   constexpr int M = D - 1;  // marching axis
-  constexpr int W = 2;
+  constexpr int W = Sh::W;
 
   if (sc->done) return;
   extern __shared__ __align__(128) unsigned char pack_smem_raw[];
@@ -78,7 +94,7 @@ __global__ void __launch_bounds__(PackShape<D, NWX, TY, NH>::NT, MINB)
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int nx = g.n[0], ny = g.n[1], nM = g.n[M];
   constexpr int bnd = BND;
-  const int x0 = blockIdx.x * TXC;
+  const int x0 = blockIdx.x * Sh::TXO - Sh::GH;  // global x of tile column 0 (NH = 0: a ghost cell)
   const int y0 = (D == 3) ? blockIdx.y * TY : 0;
   const int bm = (D == 3) ? blockIdx.z : blockIdx.y;
   const int m0 = bm * depth;
@@ -88,12 +104,12 @@ __global__ void __launch_bounds__(PackShape<D, NWX, TY, NH>::NT, MINB)
   auto plane_of = [&](int m) { return map_index(m, nM, bnd) * psi; };
   auto grid_row = [&](int gj) { return (D == 3) ? march_src(gj, ny, bnd) * nx : 0; };
   // the W cells of a CellSrc: one 8-byte load when they are known to be a pair
-  auto ldg_pair = [&](const float* __restrict__ A, int base, const CellSrc& c) {
-    if constexpr (BND == BOUNDARY_PERIODIC) return f32x2(__ldg(reinterpret_cast<const float2*>(A + (base + c.o0))));
+  auto ldg_pair = [&](const S* __restrict__ A, int base, const CellSrc& c) {
+    if constexpr (W == 2 && BND == BOUNDARY_PERIODIC) return f32x2(__ldg(reinterpret_cast<const float2*>(A + (base + c.o0))));
     else return ldg_cells<T>(A, base, c);
   };
 
-  float s_max = 0.0f;
+  S s_max = S(0);
   int bad = 0;
 
   if (warp < NWX * TY) {
@@ -104,7 +120,7 @@ __global__ void __launch_bounds__(PackShape<D, NWX, TY, NH>::NT, MINB)
     const int gi = x0 + c0;
     const int gj = y0 + row;
     const int pc = c0 + 2, pr = row + OY;
-    const bool active = gi < nx && (D == 2 || gj < ny);
+    const bool active = gi < nx && (D == 2 || gj < ny) && c0 >= Sh::GH && c0 < TXC - Sh::GH;
     const CellSrc src = cell_src<T>(gi, grid_row(gj), nx, bnd);
     const int own = (D == 3 ? gj * nx : 0) + gi;
 
@@ -119,7 +135,7 @@ __global__ void __launch_bounds__(PackShape<D, NWX, TY, NH>::NT, MINB)
       const int pl = plane_of(mi);
 #pragma unroll
       for (int f = 0; f < NF; ++f) {
-        if constexpr (BND == BOUNDARY_PERIODIC) {
+        if constexpr (W == 1 || BND == BOUNDARY_PERIODIC) {
           cp_async8(&sm.Un[f][row][c0], Uin + (f * Ni + pl + src.o0));
         } else {
           cp_async4(&sm.Un[f][row][c0], Uin + (f * Ni + pl + src.o0));
@@ -128,9 +144,9 @@ __global__ void __launch_bounds__(PackShape<D, NWX, TY, NH>::NT, MINB)
         if (active && cell >= 0) cp_async8(&sm.Ub[f][row][c0], Ubase + (f * Ni + cell));
       }
     };
-    const float lam0 = float(sc->lam[STAGE - 1][0]);
-    const float lam1 = float(sc->lam[STAGE - 1][1]);
-    const float lam2 = (D == 3) ? float(sc->lam[STAGE - 1][2]) : 0.0f;
+    const S lam0 = S(sc->lam[STAGE - 1][0]);
+    const S lam1 = S(sc->lam[STAGE - 1][1]);
+    const S lam2 = (D == 3) ? S(sc->lam[STAGE - 1][2]) : S(0);
 
     // ---- prologue: planes m0, m0+1 of the ring, the high-side state of plane m0 and the flux through face m0-1/2
     {
@@ -188,9 +204,9 @@ __global__ void __launch_bounds__(PackShape<D, NWX, TY, NH>::NT, MINB)
           sts(&sm.V[s2][f][pr][pc], vp2[f]);
           const T vp1 = lds<T>(&sm.V[s1][f][pr][pc]);
           const T dy = minbee_dy(vc[f], vp1, vp2[f]);
-          loM1[f] = rfma(-0.5f, dy, vp1);
+          loM1[f] = rfma(S(-0.5), dy, vp1);
           hiM[f] = lds<T>(&sm.Hm[f][row][c0]);
-          sts(&sm.Hm[f][row][c0], rfma(0.5f, dy, vp1));
+          sts(&sm.Hm[f][row][c0], rfma(S(0.5), dy, vp1));
         }
         T Fn[NF];
         riemann_flux<T, D, M, RS>(g.gamma, g.igm1, prim_from_fields<T, D>(hiM), prim_from_fields<T, D>(loM1), Fn);
@@ -209,17 +225,17 @@ __global__ void __launch_bounds__(PackShape<D, NWX, TY, NH>::NT, MINB)
         const T l = xshift_left(vc[f], sm.V[s0][f][pr][pc - 1]);
         const T r = xshift_right(vc[f], sm.V[s0][f][pr][pc + W]);
         const T dy = minbee_dy(l, vc[f], r);
-        const T lox = rfma(-0.5f, dy, vc[f]);
-        hix[f] = rfma(0.5f, dy, vc[f]);
-        if (lane == 0) sm.LOx[f][row][wx] = lox.v.x;
-        rs[f] = xshift_right(lox, shfl_dn(lox.v.x));
+        const T lox = rfma(S(-0.5), dy, vc[f]);
+        hix[f] = rfma(S(0.5), dy, vc[f]);
+        if (lane == 0) sm.LOx[f][row][wx] = lane_first(lox);
+        rs[f] = xshift_right(lox, shfl_dn(lane_first(lox)));
       }
       if constexpr (D == 3) {
 #pragma unroll
         for (int f = 0; f < NF; ++f) {
           const T dy = minbee_dy(lds<T>(&sm.V[s0][f][pr - 1][pc]), vc[f], lds<T>(&sm.V[s0][f][pr + 1][pc]));
-          sts(&sm.LOy[f][row][c0], rfma(-0.5f, dy, vc[f]));
-          hiy[f] = rfma(0.5f, dy, vc[f]);
+          sts(&sm.LOy[f][row][c0], rfma(S(-0.5), dy, vc[f]));
+          hiy[f] = rfma(S(0.5), dy, vc[f]);
         }
       }
       };
@@ -231,12 +247,12 @@ __global__ void __launch_bounds__(PackShape<D, NWX, TY, NH>::NT, MINB)
       T Fx[NF], Fy[(D == 3) ? NF : 1];
       if (lane == 31) {
 #pragma unroll
-        for (int f = 0; f < NF; ++f) rs[f].v.y = sm.LOx[f][row][wx + 1];
+        for (int f = 0; f < NF; ++f) lane_set_last(rs[f], sm.LOx[f][row][wx + 1]);
       }
       riemann_flux<T, D, 0, RS>(g.gamma, g.igm1, prim_from_fields<T, D>(hix), prim_from_fields<T, D>(rs), Fx);
       if (NWX > 1 && lane == 31 && wx + 1 < NWX) {
 #pragma unroll
-        for (int f = 0; f < NF; ++f) sm.Fx[f][row][wx + 1] = Fx[f].v.y;
+        for (int f = 0; f < NF; ++f) sm.Fx[f][row][wx + 1] = lane_last(Fx[f]);
       }
       if constexpr (D == 3) {
         T a[NF];
@@ -254,7 +270,7 @@ __global__ void __launch_bounds__(PackShape<D, NWX, TY, NH>::NT, MINB)
       T lowx[NF];
 #pragma unroll
       for (int f = 0; f < NF; ++f) {
-        float nb = shfl_up(Fx[f].v.y);
+        S nb = shfl_up(lane_last(Fx[f]));
         if (lane == 0) nb = sm.Fx[f][row][wx];
         lowx[f] = xshift_left(Fx[f], nb);
       }
@@ -274,7 +290,7 @@ __global__ void __launch_bounds__(PackShape<D, NWX, TY, NH>::NT, MINB)
         }
         if (STAGE == 2 && g.integrator == 1) {  // Heun: U2 = 0.5 (U0 + (U1 + dt L(U1))); U0 still sits in Uout
 #pragma unroll
-          for (int f = 0; f < NF; ++f) u[f] = 0.5f * (ld_cells_rw<T>(Uout, f * Ni + cell) + u[f]);
+          for (int f = 0; f < NF; ++f) u[f] = S(0.5) * (ld_cells_rw<T>(Uout, f * Ni + cell) + u[f]);
         }
 #pragma unroll
         for (int f = 0; f < NF; ++f) st_cells<T>(Uout, f * Ni + cell, u[f]);
@@ -290,7 +306,7 @@ __global__ void __launch_bounds__(PackShape<D, NWX, TY, NH>::NT, MINB)
       s1 = s2;
       s2 = t;
     }
-  } else {
+  } else if constexpr (NH > 0) {
     // =========================================================================== the halo warp
     // Loads the 2-cell star halo of every plane, converts it to primitives (into the ring slot of the NEXT plane) and
     // computes the faces the tile cannot get from its own cells.  NH = 2: the first halo warp serves the y direction
@@ -299,7 +315,7 @@ __global__ void __launch_bounds__(PackShape<D, NWX, TY, NH>::NT, MINB)
     const int hw = warp - NWX * TY;
     const bool do_y = (D == 3) && (NH == 1 || hw == 0);
     const bool do_x = (NH == 1 || hw == NH - 1);
-    constexpr int XHALO = 2 * XROWS;                    // x halo pairs per plane: rows x {left pair, right pair}
+    constexpr int XHALO = 4 * XROWS / W;                // x halo slots per plane: rows x {2 cells left, 2 cells right} / W
     constexpr int NXP = (XHALO + 31) / 32;
     CellSrc hsrc[NXP];
     int hpy[NXP], hpx[NXP];
@@ -308,8 +324,8 @@ __global__ void __launch_bounds__(PackShape<D, NWX, TY, NH>::NT, MINB)
     for (int q = 0; q < NXP; ++q) {
       const int id = lane + 32 * q;
       hval[q] = do_x && id < XHALO;
-      const int r = hval[q] ? (id >> 1) : 0;
-      const int px = (id & 1) ? TXC + 2 : 0;
+      const int r = hval[q] ? (W == 2 ? (id >> 1) : (id >> 2)) : 0;
+      const int px = (W == 2) ? ((id & 1) ? TXC + 2 : 0) : ((id & 3) < 2 ? (id & 3) : TXC + (id & 3));
       hpy[q] = r + OY;
       hpx[q] = px;
       hsrc[q] = cell_src<T>(x0 + px - 2, grid_row(y0 + r), nx, bnd);
@@ -354,14 +370,14 @@ __global__ void __launch_bounds__(PackShape<D, NWX, TY, NH>::NT, MINB)
       }
     };
     // x face tasks: lane l handles tile rows ra (first lane of T) and rb (second lane)
-    constexpr int XTASK_LANES = (XROWS + 1) / 2;
+    constexpr int XTASK_LANES = (XROWS + W - 1) / W;
     const bool xtask = do_x && lane < XTASK_LANES;
     const int ra = xtask ? lane : 0;
-    const int rb = min(ra + XTASK_LANES, XROWS - 1);
+    const int rb = (W == 2) ? min(ra + XTASK_LANES, XROWS - 1) : ra;
     auto plane_x = [&](int s, int qx) {
       T u[NF];
 #pragma unroll
-      for (int f = 0; f < NF; ++f) u[f] = T(sm.V[s][f][ra + OY][qx], sm.V[s][f][rb + OY][qx]);
+      for (int f = 0; f < NF; ++f) u[f] = lane_pack(sm.V[s][f][ra + OY][qx], sm.V[s][f][rb + OY][qx], (T*)nullptr);
       return prim_from_fields<T, D>(u);
     };
     auto plane_y = [&](int s, int py) {
@@ -399,8 +415,8 @@ __global__ void __launch_bounds__(PackShape<D, NWX, TY, NH>::NT, MINB)
         prim_to_fields<T, D>(lo, a);
 #pragma unroll
         for (int f = 0; f < NF; ++f) {
-          sm.LOx[f][ra][NWX] = a[f].v.x;
-          sm.LOx[f][rb][NWX] = a[f].v.y;
+          sm.LOx[f][ra][NWX] = lane_first(a[f]);
+          if (W == 2) sm.LOx[f][rb][NWX] = lane_last(a[f]);
         }
       }
       if (more) store_halo(s1);
@@ -417,12 +433,12 @@ __global__ void __launch_bounds__(PackShape<D, NWX, TY, NH>::NT, MINB)
       if (xtask) {
         T a[NF], F[NF];
 #pragma unroll
-        for (int f = 0; f < NF; ++f) a[f] = T(sm.LOx[f][ra][0], sm.LOx[f][rb][0]);
+        for (int f = 0; f < NF; ++f) a[f] = lane_pack(sm.LOx[f][ra][0], sm.LOx[f][rb][0], (T*)nullptr);
         riemann_flux<T, D, 0, RS>(g.gamma, g.igm1, hiXlow, prim_from_fields<T, D>(a), F);
 #pragma unroll
         for (int f = 0; f < NF; ++f) {
-          sm.Fx[f][ra][0] = F[f].v.x;
-          sm.Fx[f][rb][0] = F[f].v.y;
+          sm.Fx[f][ra][0] = lane_first(F[f]);
+          if (W == 2) sm.Fx[f][rb][0] = lane_last(F[f]);
         }
       }
       if (m + 2 < m1) load_halo(m + 2);
@@ -435,27 +451,52 @@ __global__ void __launch_bounds__(PackShape<D, NWX, TY, NH>::NT, MINB)
   }
   if (STAGE == 2) {
     const unsigned int nblocks = gridDim.x * gridDim.y * gridDim.z;
-    block_reduce_and_finalize<float>(s_max, bad, sc, g, nblocks, 1);
+    block_reduce_and_finalize<S>(s_max, bad, sc, g, nblocks, 1);
   }
 }
 
 // ------------------------------------------------------------------------------------------------
-template <int D, int RS, int STAGE, int NWX, int TY, int MINB, int BND, int NH>
-static bool launch_pack_bnd(const float* Uin, const float* Ubase, float* Uout, const Geom<float>& g, Scalars* sc,
-                            cudaStream_t stream, int depth) {
-  using Sh = PackShape<D, NWX, TY, NH>;
-  auto kern = k_pack<D, RS, STAGE, NWX, TY, MINB, BND, NH>;
-  static bool configured[64] = {};
+// Planes marched per block when the caller gives none.  A block pays a prologue of about two planes' work, and the
+// grid runs in waves of `capacity` blocks: the depth (8 .. 128) is the one that wastes least of both, i.e. maximises
+// (blocks / (waves * capacity)) * depth / (depth + 2); ties go to the deeper march.
+inline int pack_default_depth(long long tiles_in_plane, int nM, int capacity) {
+  int best = 8;
+  double best_eff = -1.0;
+  for (int zb = (nM + 127) / 128; zb <= (nM + 7) / 8; ++zb) {
+    const int depth = (nM + zb - 1) / zb;
+    const long long blocks = tiles_in_plane * ((nM + depth - 1) / depth);
+    const long long waves = (blocks + capacity - 1) / capacity;
+    const double eff = double(blocks) / double(waves * capacity) * depth / (depth + 2.0);
+    if (eff > best_eff * 1.0001) {
+      best_eff = eff;
+      best = depth;
+    }
+  }
+  return best;
+}
+
+template <class T, int D, int RS, int STAGE, int NWX, int TY, int MINB, int BND, int NH>
+static bool launch_pack_bnd(const scalar_t<T>* Uin, const scalar_t<T>* Ubase, scalar_t<T>* Uout, const Geom<scalar_t<T>>& g,
+                            Scalars* sc, cudaStream_t stream, int depth) {
+  using Sh = PackShape<T, D, NWX, TY, NH>;
+  auto kern = k_pack<T, D, RS, STAGE, NWX, TY, MINB, BND, NH>;
+  static int capacity[64] = {};  // blocks of this kernel the whole device holds at once (0: not configured yet)
   int dev = 0;
   if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return false;
-  if (!configured[dev]) {
+  if (!capacity[dev]) {
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(typename Sh::Smem)) != cudaSuccess)
       return false;
-    configured[dev] = true;
+    int per_sm = 0, sms = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, Sh::NT, sizeof(typename Sh::Smem)) != cudaSuccess ||
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || per_sm < 1 || sms < 1)
+      return false;
+    capacity[dev] = per_sm * sms;
   }
   constexpr int M = D - 1;
   dim3 grid, block(Sh::NT, 1, 1);
-  grid.x = (g.n[0] + Sh::TXC - 1) / Sh::TXC;
+  grid.x = (g.n[0] + Sh::TXO - 1) / Sh::TXO;
+  if (depth <= 0)
+    depth = pack_default_depth((long long)grid.x * (D == 3 ? (g.n[1] + TY - 1) / TY : 1), g.n[M], capacity[dev]);
   if (D == 3) {
     grid.y = (g.n[1] + TY - 1) / TY;
     grid.z = (g.n[M] + depth - 1) / depth;
@@ -469,47 +510,78 @@ static bool launch_pack_bnd(const float* Uin, const float* Ubase, float* Uout, c
   return true;
 }
 
-template <int D, int RS, int STAGE, int NWX, int TY, int MINB, int NH = 1>
-static bool launch_pack_shape(const float* Uin, const float* Ubase, float* Uout, const Geom<float>& g, Scalars* sc,
-                              cudaStream_t stream, int depth) {
+template <class T, int D, int RS, int STAGE, int NWX, int TY, int MINB, int NH = 1>
+static bool launch_pack_shape(const scalar_t<T>* Uin, const scalar_t<T>* Ubase, scalar_t<T>* Uout, const Geom<scalar_t<T>>& g,
+                              Scalars* sc, cudaStream_t stream, int depth) {
   if (g.boundary == BOUNDARY_PERIODIC)
-    return launch_pack_bnd<D, RS, STAGE, NWX, TY, MINB, BOUNDARY_PERIODIC, NH>(Uin, Ubase, Uout, g, sc, stream, depth);
-  return launch_pack_bnd<D, RS, STAGE, NWX, TY, MINB, BOUNDARY_OUTFLOW, NH>(Uin, Ubase, Uout, g, sc, stream, depth);
+    return launch_pack_bnd<T, D, RS, STAGE, NWX, TY, MINB, BOUNDARY_PERIODIC, NH>(Uin, Ubase, Uout, g, sc, stream, depth);
+  return launch_pack_bnd<T, D, RS, STAGE, NWX, TY, MINB, BOUNDARY_OUTFLOW, NH>(Uin, Ubase, Uout, g, sc, stream, depth);
 }
 
-// Returns false when the packed kernel does not cover this shape (odd n_x, unknown block shape): the caller falls back.
+// Returns false when the packed kernel does not cover this shape (fp32: odd n_x; unknown block shape): the caller falls back.
 //   block[0] (2-D): main warps per block (0 = default); block[1] (3-D): main warps TY (0 = default; 14 = two halo warps)
-template <int D, int RS, int STAGE>
-bool launch_pack_stage(const float* Uin, const float* Ubase, float* Uout, const Geom<float>& g, Scalars* sc,
-                       cudaStream_t stream, const int* block, int tile_depth) {
+// Real = float: T = f32x2 (two cells per thread); Real = double: T = double (one cell per thread, same 8 bytes).
+template <class Real, int D, int RS, int STAGE>
+bool launch_pack_stage(const Real* Uin, const Real* Ubase, Real* Uout, const Geom<Real>& g, Scalars* sc, cudaStream_t stream,
+                       const int* block, int tile_depth) {
   if constexpr (D == 1) {
     return false;
   } else {
-    if (g.n[0] % 2 != 0) return false;
+    constexpr bool F32 = sizeof(Real) == 4;
+    using T = typename std::conditional<F32, f32x2, double>::type;
+    constexpr int W = LaneTraits<T>::W;
+    if (W == 2 && g.n[0] % 2 != 0) return false;
     if constexpr (D == 2) {
-      const int nwx = block[0] > 0 ? block[0] : 4;
-      const long long tiles = (g.n[0] + nwx * 64 - 1) / (nwx * 64);
-      const int depth = tile_depth > 0 ? tile_depth : march_default_depth(tiles, g.n[1]);
-      if (nwx == 2) return launch_pack_shape<D, RS, STAGE, 2, 1, 2>(Uin, Ubase, Uout, g, sc, stream, depth);
-      if (nwx == 4) return launch_pack_shape<D, RS, STAGE, 4, 1, 2>(Uin, Ubase, Uout, g, sc, stream, depth);
-      if (nwx == 7) return launch_pack_shape<D, RS, STAGE, 7, 1, 2>(Uin, Ubase, Uout, g, sc, stream, depth);
+      // 2-D rows: overlapping tiles, no halo warp (block[2] = 1: the halo-warp form of the same kernel).  Default
+      // row width: the one of 2 / 4 / 8 warps that leaves the fewest idle lanes (ghost cells + ragged last tile)
+      const bool halo_warp = block[2] == 1;
+      int nwx = block[0];
+      if (nwx <= 0) {
+        double best = -1.0;
+        for (int c : {2, 4, 8}) {
+          const int owned = c * 32 * W - 4;
+          // lanes at work; wider rows pay more for their block barriers (measured: 2 warps beat 4 at equal lane use)
+          const double eff = double(g.n[0]) / double((long long)((g.n[0] + owned - 1) / owned) * c * 32 * W) *
+                             (c == 2 ? 1.0 : (c == 4 ? 0.97 : 0.94));
+          if (eff > best * 1.0001) {
+            best = eff;
+            nwx = c;
+          }
+        }
+        if (halo_warp) nwx = 4;
+      }
+      const int depth = tile_depth;  // 0: launch_pack_bnd picks it from the kernel's occupancy
+      constexpr int MB = F32 ? 2 : PH_PACK64_MINB2;
+      if (!halo_warp) {
+        if constexpr (F32)
+          if (nwx == 1) return launch_pack_shape<T, D, RS, STAGE, 1, 1, MB, 0>(Uin, Ubase, Uout, g, sc, stream, depth);
+        if (nwx == 2) return launch_pack_shape<T, D, RS, STAGE, 2, 1, MB, 0>(Uin, Ubase, Uout, g, sc, stream, depth);
+        if (nwx == 4) return launch_pack_shape<T, D, RS, STAGE, 4, 1, MB, 0>(Uin, Ubase, Uout, g, sc, stream, depth);
+        if (nwx == 8) return launch_pack_shape<T, D, RS, STAGE, 8, 1, MB, 0>(Uin, Ubase, Uout, g, sc, stream, depth);
+        return false;
+      }
+      if (nwx == 2) return launch_pack_shape<T, D, RS, STAGE, 2, 1, MB>(Uin, Ubase, Uout, g, sc, stream, depth);
+      if (nwx == 4) return launch_pack_shape<T, D, RS, STAGE, 4, 1, MB>(Uin, Ubase, Uout, g, sc, stream, depth);
+      if (nwx == 7) return launch_pack_shape<T, D, RS, STAGE, 7, 1, MB>(Uin, Ubase, Uout, g, sc, stream, depth);
       return false;
     } else {
       // default tile height: 14 rows + two halo warps (one block of 16 warps per SM: the halo work per cell halves and
       // neither halo warp has more work per plane than a main warp) when the grid gives every SM several such blocks
       // at the full marching depth; 7 rows + one halo warp (two blocks per SM) otherwise (profiles/r2_README.md)
       int ty = block[1];
+      const int tw = 32 * W;
       if (ty <= 0) {
-        const long long tiles14 = (long long)((g.n[0] + 63) / 64) * ((g.n[1] + 13) / 14);
+        const long long tiles14 = (long long)((g.n[0] + tw - 1) / tw) * ((g.n[1] + 13) / 14);
         ty = tiles14 * ((g.n[2] + 127) / 128) >= 4 * 148 ? 14 : 7;
       }
-      const long long tiles = (long long)((g.n[0] + 63) / 64) * ((g.n[1] + ty - 1) / ty);
-      const int depth = tile_depth > 0 ? tile_depth : march_default_depth(tiles, g.n[2]);
-      if (ty == 7) return launch_pack_shape<D, RS, STAGE, 1, 7, 2>(Uin, Ubase, Uout, g, sc, stream, depth);
-      if (ty == 5) return launch_pack_shape<D, RS, STAGE, 1, 5, 2>(Uin, Ubase, Uout, g, sc, stream, depth);
-      if (ty == 11) return launch_pack_shape<D, RS, STAGE, 1, 11, 1>(Uin, Ubase, Uout, g, sc, stream, depth);
-      if (ty == 15) return launch_pack_shape<D, RS, STAGE, 1, 15, 1>(Uin, Ubase, Uout, g, sc, stream, depth);
-      if (ty == 14) return launch_pack_shape<D, RS, STAGE, 1, 14, 1, 2>(Uin, Ubase, Uout, g, sc, stream, depth);
+      const int depth = tile_depth;  // 0: launch_pack_bnd picks it from the kernel's occupancy
+      if (ty == 7) return launch_pack_shape<T, D, RS, STAGE, 1, 7, 2>(Uin, Ubase, Uout, g, sc, stream, depth);
+      if (ty == 14) return launch_pack_shape<T, D, RS, STAGE, 1, 14, 1, 2>(Uin, Ubase, Uout, g, sc, stream, depth);
+      if constexpr (F32) {
+        if (ty == 5) return launch_pack_shape<T, D, RS, STAGE, 1, 5, 2>(Uin, Ubase, Uout, g, sc, stream, depth);
+        if (ty == 11) return launch_pack_shape<T, D, RS, STAGE, 1, 11, 1>(Uin, Ubase, Uout, g, sc, stream, depth);
+        if (ty == 15) return launch_pack_shape<T, D, RS, STAGE, 1, 15, 1>(Uin, Ubase, Uout, g, sc, stream, depth);
+      }
       return false;
     }
   }

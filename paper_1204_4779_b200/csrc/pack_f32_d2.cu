@@ -4,7 +4,7 @@
 
 namespace ph {
 #define PH_INST(RS, STAGE)                                                                                       \
-  template bool launch_pack_stage<2, RS, STAGE>(const float*, const float*, float*, const Geom<float>&, Scalars*, \
+  template bool launch_pack_stage<float, 2, RS, STAGE>(const float*, const float*, float*, const Geom<float>&, Scalars*, \
                                                 cudaStream_t, const int*, int);
 PH_INST(RIEMANN_HLLC, 1)
 PH_INST(RIEMANN_HLLC, 2)

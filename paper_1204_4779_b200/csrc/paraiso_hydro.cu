@@ -34,12 +34,20 @@ PH_EXTERN(double, 2)
 PH_EXTERN(double, 3)
 #undef PH_EXTERN
 #undef PH_EXTERN1
-// the packed fp32 kernels live in pack_f32_d<D>.cu
-#define PH_EXTERN_PACK(DD, RS, ST)                                                                             \
-  extern template bool launch_pack_stage<DD, RS, ST>(const float*, const float*, float*, const Geom<float>&, \
-                                                     Scalars*, cudaStream_t, const int*, int);
-PH_EXTERN_PACK(2, RIEMANN_HLLC, 1) PH_EXTERN_PACK(2, RIEMANN_HLLC, 2) PH_EXTERN_PACK(2, RIEMANN_HLL, 1) PH_EXTERN_PACK(2, RIEMANN_HLL, 2)
-PH_EXTERN_PACK(3, RIEMANN_HLLC, 1) PH_EXTERN_PACK(3, RIEMANN_HLLC, 2) PH_EXTERN_PACK(3, RIEMANN_HLL, 1) PH_EXTERN_PACK(3, RIEMANN_HLL, 2)
+// the packed / shared-memory-window kernels live in pack_f<32|64>_d<D>.cu
+#define PH_EXTERN_PACK1(REAL, DD, RS, ST)                                                                              \
+  extern template bool launch_pack_stage<REAL, DD, RS, ST>(const REAL*, const REAL*, REAL*, const Geom<REAL>&, Scalars*, \
+                                                           cudaStream_t, const int*, int);
+#define PH_EXTERN_PACK(REAL, DD)             \
+  PH_EXTERN_PACK1(REAL, DD, RIEMANN_HLLC, 1) \
+  PH_EXTERN_PACK1(REAL, DD, RIEMANN_HLLC, 2) \
+  PH_EXTERN_PACK1(REAL, DD, RIEMANN_HLL, 1)  \
+  PH_EXTERN_PACK1(REAL, DD, RIEMANN_HLL, 2)
+PH_EXTERN_PACK(float, 2)
+PH_EXTERN_PACK(float, 3)
+PH_EXTERN_PACK(double, 2)
+PH_EXTERN_PACK(double, 3)
+#undef PH_EXTERN_PACK1
 #undef PH_EXTERN_PACK
 }  // namespace ph
 
@@ -275,10 +283,9 @@ struct Launch {
   static void on_chip_stage(paraiso_hydro* h, const Geom<Real>& g, const Real* Uin, Real* Uout) {
     const Real* base = stage_base<STAGE>(h);
     auto try_pack = [&]() -> bool {
-      if constexpr (sizeof(Real) == 4 && D >= 2) {
+      if constexpr (D >= 2) {
         if (h->cells_per_thread == 0 && h->staging == 0 && h->arith == 0 &&
-            launch_pack_stage<D, RS, STAGE>((const float*)Uin, (const float*)base, (float*)Uout, g, h->sc, h->stream,
-                                            h->block, h->tile_depth)) {
+            launch_pack_stage<Real, D, RS, STAGE>(Uin, base, Uout, g, h->sc, h->stream, h->block, h->tile_depth)) {
           h->kernel_used = KERNEL_PACK;
           return true;
         }
@@ -318,15 +325,11 @@ struct Launch {
       default: {  // VARIANT_FUSED: the fastest on-chip kernel per grid kind (profiles/r2_tune_*.txt)
         if (D == 1) {
           ok = try_delayed();
-        } else if (sizeof(Real) == 4) {
-          // fp32: the packed kernel (even n_x); the options only k_march knows (cells_per_thread, staging, arith)
-          // select k_march
+        } else {
+          // the shared-memory-window kernel k_pack (fp32: packed pairs, even n_x; fp64: one cell per thread); the
+          // options only k_march knows (cells_per_thread, staging, arith) select k_march
           const bool march_only = h->cells_per_thread || h->staging || h->arith;
           ok = march_only ? try_march() : (try_pack() || try_march());
-        } else if (D == 2) {
-          ok = try_fused1();
-        } else {
-          ok = try_march();
         }
         if (!ok && !shaped) ok = try_march() || try_fused1() || try_delayed();
       }

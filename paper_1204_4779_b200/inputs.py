@@ -170,4 +170,8 @@ def baseline_config(i, scale=1.0):
         return blast(s(256), np.float32, seed=2, steps=50)
     if i == 4:
         return blast(s(512), np.float32, seed=3, steps=20)
+    if i == 11:  # not a BASELINE config: config 1's recipe at 4096^2 (fp32), the 2-D fp32 case that is NOT L2-resident
+        return kelvin_helmholtz(s(4096), dtype=np.float32, seed=0, steps=50)
+    if i == 13:  # not a BASELINE config: config 3's recipe in fp64 (the 3-D fp64 case)
+        return blast(s(256), np.float64, seed=2, steps=20)
     raise ValueError(i)

@@ -33,7 +33,7 @@ def covers(variant, dims, dtype, n):
     if variant in ("march", "fused1"):
         return dims >= 2
     if variant == "pack":
-        return dims >= 2 and np.dtype(dtype) == np.float32 and n[0] % 2 == 0
+        return dims >= 2 and (np.dtype(dtype) == np.float64 or n[0] % 2 == 0)  # fp32: pairs of cells, even n_x
     return True
 
 
@@ -102,7 +102,7 @@ def test_hundred_steps_match_oracle(gpu, oracle_mod, variant, dims, dtype):
 @pytest.mark.parametrize("n", [(4,), (5,), (4, 4), (4, 7), (4, 4, 4), (6, 4, 5), (66, 9, 4)])
 def test_minimum_size_grids(gpu, oracle_mod, variant, n):
     """n_a = 4 is the smallest legal periodic axis (stencil reach 2): every halo wraps onto the tile itself."""
-    dtype = np.float32 if variant == "pack" else np.float64
+    dtype = np.float32 if variant == "pack" and n[0] % 2 == 0 else np.float64
     if not covers(variant, len(n), dtype, n):
         pytest.skip("kernel does not cover this grid kind")
     for boundary in ("periodic", "outflow"):
@@ -267,9 +267,11 @@ def test_march_launch_shapes_match_oracle(gpu, oracle_mod, dims, opts, boundary)
         assert np.array_equal(got, ref), "the marching kernel states the same arithmetic as the oracle: bit-equal"
 
 
-# every launch shape of the packed kernel (variant pack): 2-D rows of 2 / 4 / 7 warps, 3-D tiles of 5 / 7 / 11 / 15 rows
-# with one halo warp and of 14 rows with two (one for the y faces, one for the x faces)
-PACK_SHAPES = [(2, {"block_x": 2}), (2, {"block_x": 4, "tile_depth": 5}), (2, {"block_x": 7}),
+# every launch shape of the packed kernel (variant pack): 2-D rows of 2 / 4 / 8 warps as overlapping tiles without a halo
+# warp and rows of 2 / 4 / 7 warps with one (block_z = 1); 3-D tiles of 5 / 7 / 11 / 15 rows with one halo warp and of
+# 14 rows with two (one for the y faces, one for the x faces)
+PACK_SHAPES = [(2, {"block_x": 2}), (2, {"block_x": 4, "tile_depth": 5}), (2, {"block_x": 8}),
+               (2, {"block_x": 7, "block_z": 1}), (2, {"block_x": 4, "block_z": 1, "tile_depth": 3}),
                (3, {"block_y": 5}), (3, {"block_y": 7, "tile_depth": 3}), (3, {"block_y": 11}), (3, {"block_y": 15}),
                (3, {"block_y": 14}), (3, {"block_y": 14, "tile_depth": 4})]
 
@@ -279,13 +281,16 @@ PACK_SHAPES = [(2, {"block_x": 2}), (2, {"block_x": 4, "tile_depth": 5}), (2, {"
 def test_pack_launch_shapes_match_oracle(gpu, oracle_mod, dims, opts, boundary):
     # even n_x, ragged against every tile edge, several tiles per axis (3-D: 3 tiles in x, up to 8 in y)
     for shape in {2: [(300, 41)], 3: [(150, 37, 13), (64, 14, 9)]}[dims]:
-        w = inputs.random_smooth(shape, np.float32, seed=51 + dims, boundary=boundary)
-        ref, rdt = oracle_steps(oracle_mod, w, 3)
-        got, gdt = gpu_steps(gpu, w, 3, "pack", **opts)
-        tol1, _, toldt = TOL[np.dtype(np.float32)]
-        assert np.all(field_errors(got, ref) <= 3 * tol1), (opts, field_errors(got, ref))
-        assert all(abs(a - b) <= toldt * b for a, b in zip(gdt, rdt))
-        assert np.array_equal(got, ref), "the packed kernel states the same arithmetic as the oracle: bit-equal"
+        for dtype in (np.float32, np.float64):
+            if dtype == np.float64 and opts.get("block_y", 7) not in (7, 14):
+                continue  # fp64 (one cell per thread): 7- and 14-row tiles only
+            w = inputs.random_smooth(shape, dtype, seed=51 + dims, boundary=boundary)
+            ref, rdt = oracle_steps(oracle_mod, w, 3)
+            got, gdt = gpu_steps(gpu, w, 3, "pack", **opts)
+            tol1, _, toldt = TOL[np.dtype(dtype)]
+            assert np.all(field_errors(got, ref) <= 3 * tol1), (opts, field_errors(got, ref))
+            assert all(abs(a - b) <= toldt * b for a, b in zip(gdt, rdt))
+            assert np.array_equal(got, ref), "the packed kernel states the same arithmetic as the oracle: bit-equal"
 
 
 KERNEL_ID = {"manifest_flux": 1, "manifest_all": 2, "delayed": 3, "march": 4, "fused1": 5, "pack": 6}
@@ -324,10 +329,10 @@ def test_uncovered_shapes_are_errors(gpu, oracle_mod):
             h.set_state(w2.U)
             h.step(1e-4)
             assert h.get_option("kernel_used") == KERNEL_ID[want], (variant, h.get_option("kernel_used"))
-    with gpu.ParaisoHydro((64, 24), (1.0, 1.0), 1.4, np.float64) as h:  # 2-D fp64 default: the first fused design
+    with gpu.ParaisoHydro((64, 24), (1.0, 1.0), 1.4, np.float64) as h:  # fp64 default: the same kernel, one cell per thread
         h.set_state(inputs.random_smooth((64, 24), np.float64, seed=6).U)
         h.step(1e-4)
-        assert h.get_option("kernel_used") == KERNEL_ID["fused1"]
+        assert h.get_option("kernel_used") == KERNEL_ID["pack"]
 
 
 def test_run_reports_the_clock_when_no_step_runs(gpu):
