@@ -147,14 +147,26 @@ def oracle_rate(w, steps, warmup, threads):
 def cpu_baseline(w):
     edge = {1: 1 << 20, 2: 1536, 3: 144}[w.dims]
     s = centred_sample(w, edge)
-    r1, t1, _ = oracle_rate(s, 1, 1, "serial")
+    # the serial figure is one warm-up step, then 2 full RK2 steps (+ CFL reduction), pinned to one core
+    try:
+        allowed = os.sched_getaffinity(0)
+        os.sched_setaffinity(0, {min(allowed)})
+    except (AttributeError, OSError):
+        allowed = None
+    try:
+        r1, t1, _ = oracle_rate(s, 2, 1, "serial")
+    finally:
+        if allowed:
+            os.sched_setaffinity(0, allowed)
+    t1 /= 2.0  # seconds per serial step
     steps = max(2, int(8.0 / max(t1 / 8, 1e-3) / 8))  # ~8 s of OpenMP work if it scales, capped below
     steps = min(steps, 12)
     rn, tn, cores = oracle_rate(s, steps, 1, "omp")
     return {"value": rn, "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": f"centred {'x'.join(map(str, s.n))} sub-box of the workload's initial state, periodic, "
                       f"{steps} RK2 steps (OpenMP build of oracle/euler_oracle.cpp, bit-identical to serial)",
-            "serial_value": r1, "serial_cores": 1, "seconds": t1 * 2 + tn}
+            "serial_value": r1, "serial_cores": 1, "serial_sample": "same sub-box, 1 warm-up + 2 timed RK2 steps pinned to one core",
+            "seconds": t1 * 3 + tn}
 
 
 def reference_arm(args):
@@ -179,36 +191,66 @@ def reference_arm(args):
     print(json.dumps(line), flush=True)
 
 
-def device_run(binding, torch, w, steps, warmup, variant, riemann, per_stage, options=None):
-    """K device-paced steps with the state resident in HBM; returns dict(ms, stage_ms, stage_launches, launches)."""
+WARMUP_SECONDS = 0.5  # device work before anything is timed (clock ramp), on top of the --warmup steps
+REPEATS = 30          # every individual is scored by the mean and deviation of 30 runs
+
+
+def device_run(binding, torch, w, steps, warmup, variant, riemann, per_stage, options=None, repeats=0,
+               warmup_seconds=WARMUP_SECONDS):
+    """K device-paced steps with the state resident in HBM; returns dict(ms, stage_ms, stage_launches, launches, ...).
+
+    Warm-up: `warmup` steps, then further steps until `warmup_seconds` of device work have run (untimed); the state is
+    then set again so that the timed K steps are the first K steps of the workload.  repeats > 0: the same K-step run
+    (state set again before each) is timed `repeats` more times; their mean / sample deviation / extremes are returned
+    under "repeats" (the headline stays the first run, as the bench contract words it)."""
     s = torch.cuda.Stream()
     with binding.ParaisoHydro(w.n, w.extent, w.gamma, w.dtype, w.boundary, riemann, variant, stream=s,
                               **(options or {})) as h:
         dev = torch.from_numpy(w.U).cuda()
         h.set_state(dev)
-        del dev
         h.run(w.cfl, warmup)
         h.sync()
-        if per_stage:
-            h.kernel_time(1)
-        l0 = h.launch_count()
+        t_w = time.perf_counter()
+        chunk = max(1, min(steps, 8))
+        while time.perf_counter() - t_w < warmup_seconds:
+            h.run(w.cfl, chunk)
+            h.sync()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        torch.cuda.synchronize()
-        e0.record(s)
-        h.run(w.cfl, steps)
-        e1.record(s)
-        e1.synchronize()
-        torch.cuda.synchronize()
-        ms = e0.elapsed_time(e1)
+
+        def timed(first):
+            h.set_state(dev)  # device source: stays alive until the handle is closed (the copy is asynchronous)
+            h.run(w.cfl, warmup)
+            h.sync()
+            if first and per_stage:
+                h.kernel_time(1)
+            torch.cuda.synchronize()
+            counted[0] = h.launch_count()
+            e0.record(s)
+            h.run(w.cfl, steps)
+            e1.record(s)
+            e1.synchronize()
+            torch.cuda.synchronize()
+            counted[1] = h.launch_count()
+            return e0.elapsed_time(e1)
+
+        counted = [0, 0]  # the library's launch counter before / after the timed region
+        ms = timed(True)
+        launches = counted[1] - counted[0]
         stage_ms, stage_n = h.kernel_time() if per_stage else (ms, 2 * steps)
-        if per_stage:
+        if per_stage:  # the warm-up steps of timed() ran before the stage clock was switched on
             h.kernel_time(0)
-        launches = h.launch_count() - l0
         bad = h.stats()
         t, k = h.time()
         if bad or k != steps + warmup:
             raise RuntimeError(f"bench run unhealthy: nonfinite={bad} steps={k}")
-    return {"ms": ms, "stage_ms": stage_ms, "stage_launches": stage_n, "launches": launches, "t": t}
+        rep = None
+        if repeats > 0:
+            rates = [w.cells * steps / (timed(False) * 1e-3) / 1e9 for _ in range(repeats)]
+            rep = {"n": repeats, "mean": float(np.mean(rates)), "stdev": float(np.std(rates, ddof=1)) if repeats > 1 else 0.0,
+                   "min": float(min(rates)), "max": float(max(rates)), "unit": UNIT}
+        h.sync()
+        del dev
+    return {"ms": ms, "stage_ms": stage_ms, "stage_launches": stage_n, "launches": launches, "t": t, "repeats": rep}
 
 
 def e2e_run(binding, torch, w, steps, warmup, variant, riemann):
@@ -254,7 +296,23 @@ def alu_peak_tlaneops(itemsize):
     return SM_COUNT * (128 if itemsize == 4 else 64) * SM_MAX_GHZ * 1e9 / 1e12
 
 
-def roofline_of(w, r, peak, peak_src, traffic=None):
+# arith = 1 (f32fast): an IEEE division (1 MUFU + 5) / square root (1 MUFU + 4) becomes 1 MUFU + 1 multiplication
+COUNTED_OPS_ARITH1 = {(2, 4): 638 - (27 * 4 + 9 * 3), (3, 4): 1053 - (39 * 4 + 13 * 3)}
+_MEASURED_ALU_PEAK = {}
+
+
+def measured_alu_peak(binding, itemsize):
+    """Tlaneop/s of the FFMA (fp32) / DFMA (fp64) pipe measured on this device by the probe library
+    (paraiso_probe_peak: 16 independent chains per thread, 8 warps per scheduler, best of 5), or None."""
+    if itemsize not in _MEASURED_ALU_PEAK:
+        try:
+            _MEASURED_ALU_PEAK[itemsize] = float(binding.probe_peak("ffma" if itemsize == 4 else "dfma"))
+        except Exception:
+            _MEASURED_ALU_PEAK[itemsize] = None
+    return _MEASURED_ALU_PEAK[itemsize]
+
+
+def roofline_of(w, r, peak, peak_src, traffic=None, binding=None, counted_ops=None):
     """The slower of north_star's two rooflines is the binding one and is reported as `bound`; the other is kept
     beside it.  (a) HBM: 2*nf*w*N algorithmic bytes per stage launch (state read once, written once; halo excluded)
     over the measured copy bandwidth.  (b) ALU: counted lane-operations per stage launch over the FP32 / FP64 lane
@@ -263,17 +321,23 @@ def roofline_of(w, r, peak, peak_src, traffic=None):
     nbytes = 2 * w.nf * isz * w.cells
     avg_ms = r["stage_ms"] / max(1, r["stage_launches"])
     hbm_achieved = nbytes / (avg_ms * 1e-3) / 1e9
-    ops = COUNTED_OPS_PER_CELL_STEP[(w.dims, isz)] / 2.0 * w.cells
+    counted = counted_ops or COUNTED_OPS_PER_CELL_STEP[(w.dims, isz)]
+    ops = counted / 2.0 * w.cells
     alu_achieved = ops / (avg_ms * 1e-3) / 1e12
-    alu_peak = alu_peak_tlaneops(isz)
+    alu_nominal = alu_peak_tlaneops(isz)
+    alu_measured = measured_alu_peak(binding, isz) if binding is not None else None
+    alu_peak = alu_measured or alu_nominal
     hbm = {"bound": "hbm", "achieved": hbm_achieved, "peak": peak, "unit": "GB/s", "frac": hbm_achieved / peak,
            "algorithmic_bytes_per_launch": nbytes, "peak_source": peak_src,
            "gcell_per_s_at_peak": peak * 1e9 / (4 * w.nf * isz) / 1e9}
     alu = {"bound": "alu", "achieved": alu_achieved, "peak": alu_peak, "unit": "Tlaneop/s", "frac": alu_achieved / alu_peak,
-           "algorithmic_ops_per_launch": ops, "counted_ops_per_cell_step": COUNTED_OPS_PER_CELL_STEP[(w.dims, isz)],
-           "peak_source": "derived: 148 SMs x %d %s lanes x 1.965 GHz (B200_PROFILING.md unit counts and clocks.max.sm)"
-                          % (128 if isz == 4 else 64, "FP32" if isz == 4 else "FP64"),
-           "gcell_per_s_at_peak": alu_peak * 1e12 / COUNTED_OPS_PER_CELL_STEP[(w.dims, isz)] / 1e9}
+           "algorithmic_ops_per_launch": ops, "counted_ops_per_cell_step": counted,
+           "peak_source": ("measured: %s fused multiply-adds per second on this device (paraiso_probe_peak)"
+                           % ("FFMA" if isz == 4 else "DFMA")) if alu_measured else "nominal (no probe library)",
+           "peak_nominal": alu_nominal, "frac_of_nominal": alu_achieved / alu_nominal,
+           "peak_nominal_source": "148 SMs x %d %s lanes x 1.965 GHz (B200_PROFILING.md unit counts and clocks.max.sm)"
+                                  % (128 if isz == 4 else 64, "FP32" if isz == 4 else "FP64"),
+           "gcell_per_s_at_peak": alu_peak * 1e12 / counted / 1e9}
     first, other = (alu, hbm) if alu["gcell_per_s_at_peak"] < hbm["gcell_per_s_at_peak"] else (hbm, alu)
     out = dict(first)
     out.update({"traffic": traffic, "kernel": "RK stage kernel(s) (a1-a5 [+a0 in stage 2])", "avg_launch_ms": avg_ms,
@@ -281,22 +345,31 @@ def roofline_of(w, r, peak, peak_src, traffic=None):
     return out
 
 
+_UNIT_BYTES = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
+
+
 def ncu_traffic(cfg, variant):
-    if cfg == 2 and variant == "fused":
-        variant = "fused1"  # 2-D fp64 grids: the default on-chip variant is k_fused
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, copied by hand from the
-    committed ncu --set full summary (profiles/traffic.csv names it); None if that variant was not captured."""
-    p = os.path.join(ROOT, "profiles", "traffic.csv")
+    """dram__bytes_read.sum + dram__bytes_write.sum per STAGE of the RK2 step, parsed from the committed raw ncu export
+    profiles/r2_cfg<cfg>_<variant>_ncu_raw.csv (`ncu -i ... --page raw --csv` of one `ncu --set full` capture that
+    holds exactly the kernels of ONE step, the .md beside it names the command): the sum over every captured launch
+    divided by the two stages.  For the one-kernel-per-stage variants that is the mean of the two stage launches.
+    Returns (bytes per stage, file name) or (None, None) if that configuration was not captured."""
+    import csv
+
+    name = f"r2_cfg{cfg}_{variant}_ncu_raw.csv"
+    p = os.path.join(ROOT, "profiles", name)
     if not os.path.exists(p):
-        return None
+        return None, None
     try:
-        for line in open(p).read().splitlines()[1:]:
-            key, val = line.split(",")[:2]
-            if key == f"config{cfg}:{variant}":
-                return float(val)
+        rows = list(csv.reader(open(p)))
+        hdr, units, data = rows[0], rows[1], rows[2:]
+        total = 0.0
+        for key in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+            i = hdr.index(key)
+            total += sum(float(r[i]) for r in data) * _UNIT_BYTES[units[i]]
+        return total / 2.0, name
     except Exception:
-        pass
-    return None
+        return None, None
 
 
 def replicas_aggregate(ms_local, cells, steps, world, device=None):
@@ -326,6 +399,9 @@ def main():
     ap.add_argument("--no-sweep", action="store_true", help="skip the short runs of the other configs / variants")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--repeats", type=int, default=REPEATS, help="further timed runs of the same K steps (mean +- deviation)")
+    ap.add_argument("--warmup-seconds", type=float, default=WARMUP_SECONDS,
+                    help="device work before the timed steps, on top of --warmup (0 under ncu: a fixed launch sequence)")
     ap.add_argument("--opt", action="append", default=[], help="key=value launch-shape option (block_x, ...)")
     args = ap.parse_args()
     if args.steps is None:
@@ -362,7 +438,8 @@ def main():
     barrier()
     sampler = ClockSampler(local).start() if rank == 0 else None
     t0 = time.time()
-    r = device_run(binding, torch, w, args.steps, args.warmup, args.variant, args.riemann, big, options)
+    r = device_run(binding, torch, w, args.steps, args.warmup, args.variant, args.riemann, big, options,
+                   repeats=args.repeats, warmup_seconds=args.warmup_seconds)
     t1 = time.time()
     barrier()
     clocks = sampler.stop(t0, t1) if sampler else None
@@ -376,6 +453,7 @@ def main():
                    d2h_bytes_per_step=e["d2h_bytes_per_step"] * world)
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "warmup_seconds": args.warmup_seconds,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32" if w.dtype == np.float32 else "f64", "data": "synthetic",
             "config": {"workload": f"BASELINE config {args.config}: {w.name}", "grid": list(w.n), "fields": w.nf,
@@ -383,8 +461,17 @@ def main():
                        "variant": args.variant, "options": options, "parallelism": "replicas" if world > 1 else "1gpu",
                        "l2": "state buffers (2 x %.0f MB) exceed the 126 MB L2; no flush needed" % (w.U.nbytes / 1e6)
                        if 2 * w.U.nbytes > 126e6 else "L2-RESIDENT workload (2 x %.1f MB): not an HBM number" % (w.U.nbytes / 1e6)},
-            "roofline": roofline_of(w, r, peak, peak_src, ncu_traffic(args.config, args.variant)),
+            "roofline": roofline_of(w, r, peak, peak_src, binding=binding if rank == 0 else None,
+                                    counted_ops=COUNTED_OPS_ARITH1.get((w.dims, w.dtype.itemsize)) if options.get("arith") == 1 else None),
             "e2e": e2e, "gpu_launches": r["launches"], "clocks": clocks}
+    traffic, traffic_file = ncu_traffic(args.config, args.variant) if not options else (None, None)
+    line["roofline"]["traffic"] = traffic
+    line["roofline"]["traffic_source"] = ("profiles/" + traffic_file + " (dram__bytes_read.sum + dram__bytes_write.sum of one "
+                                          "captured step / 2 stages)") if traffic_file else None
+    if r["repeats"]:
+        line["repeats"] = dict(r["repeats"], note="rank 0, per GPU: %d further runs of the same %d steps, the state set again "
+                                                   "before each (PAPER.md:626 scores by mean and deviation of 30 runs)"
+                                                   % (r["repeats"]["n"], args.steps))
 
     if rank == 0:
         # measured issue cost (scheduler cycles per instruction) of the instruction classes of the stage kernel on
@@ -403,29 +490,42 @@ def main():
 
 
 def sweep(binding, torch, args, peak, peak_src):
-    """Short runs of every BASELINE config with every kernel variant (the Manifest <-> Delayed axis), same protocol."""
+    """Short runs of every BASELINE config (and of the 4096^2 fp32 / 256^3 fp64 extras) with every kernel variant (the
+    Manifest <-> Delayed axis), same protocol: >= WARMUP_SECONDS of device work before the timed steps, each row with
+    its own clock sample."""
     out = []
-    for cfg in (0, 1, 2, 3, 4):
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    for cfg in (0, 1, 2, 3, 4, 11, 13):
         w = make_workload(cfg)
         big = w.cells >= (1 << 22)
         steps = min(DEFAULT_STEPS[cfg], 100 if not big else 10)
-        for variant in ("fused", "march", "fused1", "manifest_flux", "manifest_all", "delayed", "march arith=1"):
-            opts = None
+        for variant in ("fused", "pack", "march", "fused1", "manifest_flux", "manifest_all", "delayed", "march arith=1"):
+            opts, counted = None, None
             if variant == "march arith=1":  # fp32 only: hardware rcp / rsqrt approximations, inside the tolerances, not bit-equal
                 if w.dtype != np.float32 or w.dims == 1:
                     continue
                 opts = {"arith": 1}
+                counted = COUNTED_OPS_ARITH1[(w.dims, 4)]  # its own counted work, not the IEEE sequences'
+            if cfg in (11, 13) and variant in ("manifest_flux", "manifest_all", "delayed", "fused1"):
+                continue  # the extras are there for the on-chip kernels
+            sampler = ClockSampler(local).start()
+            t0 = time.time()
             try:
-                r = device_run(binding, torch, w, steps, 3 if w.cells >= (1 << 26) else 20, variant.split()[0], args.riemann, big, opts)
-            except Exception as ex:  # e.g. out of memory for manifest_all
+                r = device_run(binding, torch, w, steps, 3, variant.split()[0], args.riemann, big, opts)
+            except Exception as ex:  # shape not covered, out of memory for manifest_all, ...
+                sampler.stop(t0, time.time())
                 out.append({"config": cfg, "variant": variant, "error": str(ex)[:120]})
                 continue
-            rl = roofline_of(w, r, peak, peak_src)
+            clocks = sampler.stop(t0, time.time())
+            rl = roofline_of(w, r, peak, peak_src, binding=binding, counted_ops=counted)
             out.append({"config": cfg, "workload": w.name, "variant": variant, "steps": steps,
                         "value": w.cells * steps / (r["ms"] * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": r["ms"] / steps,
                         "bound": rl["bound"], "frac": rl["frac"],
                         "hbm_frac": (rl if rl["bound"] == "hbm" else rl["other_bound"])["frac"],
-                        "alu_frac": (rl if rl["bound"] == "alu" else rl["other_bound"])["frac"], "launches": r["launches"]})
+                        "alu_frac": (rl if rl["bound"] == "alu" else rl["other_bound"])["frac"],
+                        "counted_ops_per_cell_step": (rl if rl["bound"] == "alu" else rl["other_bound"])["counted_ops_per_cell_step"],
+                        "launches": r["launches"],
+                        "clocks": {"sm_mhz": clocks.get("sm_mhz"), "reasons": clocks.get("reasons")}})
         del w
     return out
 

@@ -50,6 +50,9 @@ enum {
  *   extent[dims] physical edge lengths; mesh size dr_a = extent[a] / n[a]  (Eq. 23 "Delta r_a")
  *   gamma        ratio of specific heats of the ideal-gas EOS E = p/(gamma-1) + rho v^2/2, > 1
  *   dtype        PARAISO_F32 | PARAISO_F64 — the arithmetic type of the whole path
+ * Size limit: N = prod n[a] <= 2^31 / 8 = 268 435 456 cells (645^3; 16384^2), because every kernel addresses the
+ * nf * N elements of a state buffer with 32-bit element offsets (index arithmetic is part of the issue-bound hot loop);
+ * a larger grid is EINVAL, not a wrong answer.  The five BASELINE configs need at most 512^3 = 2^27.
  * Allocates two state buffers (2 * nf * N elements) and a small scalar block on the current device.
  * Errors: EINVAL, ENOMEM, ECUDA.  *out is set only on success. */
 int paraiso_hydro_create(paraiso_hydro_t **out, int dims, const int64_t *n, const double *extent, double gamma,
@@ -62,17 +65,28 @@ int paraiso_hydro_destroy(paraiso_hydro_t *h);
  *   "boundary"  0 periodic: index wrap (default) | 1 outflow: zero-gradient, index clamp   (R12)
  *   "riemann"   0 HLLC (default; Eq. 22) | 1 HLL                              (R4)
  *   "variant"   kernel arrangement on the paper's Manifest <-> Delayed axis (Table 5):
- *               0 fused       one kernel per RK stage, intermediates on chip (default): k_march on 3-D grids and on
- *                             2-D fp32 grids, k_fused on 2-D fp64 grids, k_delayed in 1-D
- *               4 march       force k_march (halo warp + warp-shuffle exchange; "cells_per_thread" 2 = packed f32x2)
+ *               0 fused       one kernel per RK stage, intermediates on chip (default): k_pack on 2-D and 3-D grids
+ *                             (fp32: packed pairs of cells, needs an even n_x, else k_march; fp64: one cell per
+ *                             thread), k_delayed in 1-D
+ *               6 pack        force k_pack (marching window in shared memory; the fastest on-chip kernel)
+ *               4 march       force k_march (marching window in registers; "cells_per_thread" 2 = packed f32x2)
  *               5 fused1      force k_fused (the first on-chip design)
  *               1 manifest_flux  fluxes F_a materialised in HBM, then an update kernel
  *               2 manifest_all   V, VL/VR and F_a all materialised in HBM, one kernel per piece
  *               3 delayed     one kernel per stage, every thread recomputes all it needs from U
+ *               An explicitly requested kernel, or any launch-shape knob, that does not cover the grid makes the next
+ *               step / run return EINVAL ("shape not covered"); only variant 0 with all-default knobs falls back
+ *               (pack -> march -> fused1 -> delayed).  get_option("kernel_used") = the kernel of the last stage launch.
  *   "block_x" "block_y" "block_z" "tile_depth" "cells_per_thread"   launch-shape knobs of the sweep (0 = default):
- *               k_fused: block_x x block_y = tile; k_march: block_x = main warps per row (2-D), block_y = main warps
- *               (3-D), block_z = rows per main thread (3-D: 1 or 2), cells_per_thread 2 = packed f32x2;
- *               tile_depth = planes marched per block
+ *               k_pack: block_x = warps per row (2-D: 2, 4, 8 [fp32 also 1] as overlapping tiles without a halo warp;
+ *               with block_z = 1 the halo-warp form, 2, 4, 7), block_y = tile rows (3-D: 7 [default on small grids],
+ *               14 [two halo warps, default on large grids]; fp32 also 5, 11, 15); k_fused: block_x x block_y = tile;
+ *               k_march: block_x = main warps per row (2-D), block_y = main warps (3-D), block_z = rows per main
+ *               thread (3-D: 1 or 2), cells_per_thread 2 = packed f32x2; tile_depth = planes marched per block
+ *               (0: chosen from the kernel's occupancy so that the grid fills whole waves)
+ *   "limiter"   interpolation variant (R22): 0 the paper's MINBEE, Eq. 21 (default) | 1 none: piecewise
+ *               constant states, the first-order Godunov scheme | 2 monotonized central (van Leer 1977).  1 and 2 are
+ *               compile-time variants of k_pack (default launch shape only) and k_delayed; any other kernel -> EINVAL
  *   "graph"     1 replay steps of run() from a captured CUDA graph (default) | 0 plain launches
  *   "arith"     k_march, fp32 only: 0 IEEE-exact division and square root, bit-equal to the oracle (default) |
  *               1 hardware reciprocal / reciprocal-square-root approximations: inside north_star's fp32 tolerances,
@@ -92,7 +106,9 @@ int paraiso_hydro_get_option(paraiso_hydro_t *h, const char *key, int64_t *value
 int paraiso_hydro_set_stream(paraiso_hydro_t *h, void *cuda_stream);
 
 /* Copy nf*N elements of conserved variables from U (host or device) into the handle, reset t = 0 and
- * the step counter, and enqueue the standalone CFL reduction for this state. */
+ * the step counter, and enqueue the standalone CFL reduction for this state.  The copy is asynchronous on the
+ * handle's stream when U is a device pointer or pinned host memory: the caller keeps U alive (and unchanged) until the
+ * stream has passed it (paraiso_hydro_sync, or any blocking call of this handle). */
 int paraiso_hydro_set_state(paraiso_hydro_t *h, const void *U);
 
 /* Copy the current state (nf*N elements) to U_out (host or device).  Host destination: blocks until done. */
@@ -106,6 +122,19 @@ int paraiso_hydro_cfl_dt(paraiso_hydro_t *h, double cfl, double *dt_out);
 /* One full RK2 step (Eq. 24-27) with the given dt (rounded to the handle dtype; finite, > 0): t += dt.
  * Asynchronous.  The last stage also leaves S of the new state on the device. */
 int paraiso_hydro_step(paraiso_hydro_t *h, double dt);
+
+/* Prescribed ghost cells (the paper's validation runs "substitute the analytic solutions to the ghost cells",
+ * PAPER.md:846-848; R23).  In this use the outermost TWO cells of every axis of the grid are the ghost cells
+ * (two = the reach of the stencil of Eq. 20-22): the caller overwrites them with its own values, the cells in between
+ * are advanced by Eq. 23-27 as always; "boundary" should be 1 (clamp), what the scheme computes in the ghost cells
+ * themselves is overwritten before anything reads it.  G, G_mid: nf*N elements laid out like the state (host or
+ * device; same lifetime rule as set_state), of which only the ghost cells are read.
+ *   set_ghosts   ghost cells of the CURRENT state := G's (call it before every step with the ghosts of time t, and
+ *                after the last step if the ghost cells of the result matter); it does not refresh S: pass your own dt
+ *   step_ghosts  one RK2 step like paraiso_hydro_step, but the ghost cells of the intermediate state U1 := G_mid's
+ *                before the second stage (midpoint rule: the ghosts of time t + dt/2; Heun: of time t + dt) */
+int paraiso_hydro_set_ghosts(paraiso_hydro_t *h, const void *G);
+int paraiso_hydro_step_ghosts(paraiso_hydro_t *h, double dt, const void *G_mid);
 
 /* Advance with dt from the CFL condition evaluated on the device at the start of every step, without host
  * round trips: at most nsteps steps; if t_end > 0 stop when t reaches t_end, the last step clamped to land on it

@@ -12,6 +12,7 @@ from . import build as _build
 
 _LIBS = {}
 _DT = {np.dtype(np.float32): 0, np.dtype(np.float64): 1}
+LIMITER = {"minbee": 0, "none": 1, "mc": 2}
 
 
 def _lib(kind="serial"):
@@ -35,6 +36,9 @@ def _lib(kind="serial"):
         L.oracle_run.argtypes = [vp, dbl, i64, dbl, ctypes.POINTER(i64), ctypes.POINTER(dbl)]
         L.oracle_riemann.argtypes = [cint, cint, cint, cint, dbl, vp, vp, vp]
         L.oracle_minbee.argtypes = [cint, dbl, dbl, dbl, ctypes.POINTER(dbl), ctypes.POINTER(dbl)]
+        L.oracle_limited.argtypes = [cint, cint, dbl, dbl, dbl, ctypes.POINTER(dbl), ctypes.POINTER(dbl)]
+        L.oracle_set_ghosts.argtypes = [vp, vp]
+        L.oracle_step_ghosts.argtypes = [vp, dbl, vp]
         L.oracle_num_threads.restype = cint
         _LIBS[kind] = L
     return _LIBS[kind]
@@ -43,7 +47,8 @@ def _lib(kind="serial"):
 class Oracle:
     """One oracle solver instance.  State arrays are (nf, [nz,] [ny,] nx), x fastest."""
 
-    def __init__(self, n, extent, gamma, dtype, boundary="periodic", riemann="hllc", threads="serial", integrator="midpoint"):
+    def __init__(self, n, extent, gamma, dtype, boundary="periodic", riemann="hllc", threads="serial", integrator="midpoint",
+                 limiter="minbee"):
         self.n = tuple(int(v) for v in n)  # x first
         self.dims = len(self.n)
         self.dtype = np.dtype(dtype)
@@ -58,6 +63,7 @@ class Oracle:
         self._opt("boundary", {"periodic": 0, "outflow": 1}[boundary])
         self._opt("riemann", {"hllc": 0, "hll": 1}[riemann])
         self._opt("integrator", {"midpoint": 0, "heun": 1}[integrator])
+        self._opt("limiter", LIMITER[limiter])
 
     def _opt(self, key, val):
         if self._L.oracle_set_option(self._h, key.encode(), val) != 0:
@@ -89,6 +95,18 @@ class Oracle:
 
     def step(self, dt):
         self._L.oracle_step(self._h, float(dt))
+
+    def set_ghosts(self, G):
+        """Prescribed ghost cells: the outermost two cells of every axis of the current state := G's."""
+        G = np.ascontiguousarray(G, dtype=self.dtype)
+        assert G.shape == self.shape
+        self._L.oracle_set_ghosts(self._h, G.ctypes.data)
+
+    def step_ghosts(self, dt, G_mid):
+        """One RK2 step whose intermediate state gets G_mid's ghost cells before the second stage."""
+        G_mid = np.ascontiguousarray(G_mid, dtype=self.dtype)
+        assert G_mid.shape == self.shape
+        self._L.oracle_step_ghosts(self._h, float(dt), G_mid.ctypes.data)
 
     def stage(self, tau):
         out = np.empty(self.shape, self.dtype)
@@ -126,6 +144,14 @@ def riemann(VL, VR, axis, gamma, dims, dtype=np.float64, kind="hllc"):
 def minbee(y0, y1, y2, dtype=np.float64):
     lo, hi = ctypes.c_double(), ctypes.c_double()
     _lib().oracle_minbee(_DT[np.dtype(dtype)], y0, y1, y2, ctypes.byref(lo), ctypes.byref(hi))
+    return lo.value, hi.value
+
+
+def limited(limiter, y0, y1, y2, dtype=np.float64):
+    """(lo, hi) of one interpolation variant ("minbee", "none", "mc")."""
+    lo, hi = ctypes.c_double(), ctypes.c_double()
+    rc = _lib().oracle_limited(_DT[np.dtype(dtype)], LIMITER[limiter], y0, y1, y2, ctypes.byref(lo), ctypes.byref(hi))
+    assert rc == 0
     return lo.value, hi.value
 
 

@@ -50,6 +50,10 @@ namespace {
 
 enum { BOUNDARY_PERIODIC = 0, BOUNDARY_OUTFLOW = 1 };
 enum { RIEMANN_HLLC = 0, RIEMANN_HLL = 1 };
+// Interpolation variants ("interpolation methods ... combinable"): the paper's
+// MINBEE (Eq. 21, the default and what every BASELINE config runs), none (dy = 0: piecewise-constant states, the
+// first-order Godunov scheme) and the monotonized-central limiter (van Leer 1977, "MC"), an option like HLL.
+enum { LIMITER_MINBEE = 0, LIMITER_NONE = 1, LIMITER_MC = 2 };
 
 // Primitive variables V = (rho, v_a, p), Eq. 13.  Components b >= D are zero.
 template <class Real>
@@ -155,17 +159,39 @@ struct Solver {
     hi = std::fma(Real(0.5), dy, y1);   // y1 + dy/2   (face i+1/2 side)
   }
 
+  // Options beside Eq. 21 (R22), same form (lo, hi) = (y1 - dy/2, y1 + dy/2):
+  //   none: dy = 0 (the scheme degenerates to first-order Godunov, pin P10/P15)
+  //   MC  : dy = 0 if dy01 * dy12 < 0 (the same product test as Eq. 21), else the value of smallest magnitude among
+  //         2 dy01, 2 dy12 and the central difference dc = (dy01 + dy12)/2, with the sign of dc
+  static void limited(int lim, Real y0, Real y1, Real y2, Real& lo, Real& hi) {
+    if (lim == LIMITER_MINBEE) {
+      minbee(y0, y1, y2, lo, hi);
+      return;
+    }
+    Real dy = Real(0);
+    if (lim == LIMITER_MC) {
+      const Real d01 = y1 - y0;
+      const Real d12 = y2 - y1;
+      const Real dc = Real(0.5) * (d01 + d12);
+      const Real a = std::fmin(std::fmin(Real(2) * std::fabs(d01), Real(2) * std::fabs(d12)), std::fabs(dc));
+      dy = (d01 * d12 < Real(0)) ? Real(0) : std::copysign(a, dc);
+    }
+    lo = std::fma(Real(-0.5), dy, y1);
+    hi = std::fma(Real(0.5), dy, y1);
+  }
+
   // Interpolate (Eq. 20) applied to a whole primitive state, component by component.
-  static void interpolate(const Prim<Real>& V0, const Prim<Real>& V1, const Prim<Real>& V2,
-                          Prim<Real>& lo, Prim<Real>& hi) {
-    minbee(V0.rho, V1.rho, V2.rho, lo.rho, hi.rho);
+  int limiter = LIMITER_MINBEE;
+  void interpolate(const Prim<Real>& V0, const Prim<Real>& V1, const Prim<Real>& V2,
+                   Prim<Real>& lo, Prim<Real>& hi) const {
+    limited(limiter, V0.rho, V1.rho, V2.rho, lo.rho, hi.rho);
     for (int b = 0; b < 3; ++b) {
       if (b < D)
-        minbee(V0.v[b], V1.v[b], V2.v[b], lo.v[b], hi.v[b]);
+        limited(limiter, V0.v[b], V1.v[b], V2.v[b], lo.v[b], hi.v[b]);
       else
         lo.v[b] = hi.v[b] = Real(0);
     }
-    minbee(V0.p, V1.p, V2.p, lo.p, hi.p);
+    limited(limiter, V0.p, V1.p, V2.p, lo.p, hi.p);
   }
 
   // Eq. 22: flux through a face with normal e_a from the left/right primitive states.
@@ -291,6 +317,38 @@ struct Solver {
     U.swap(U2);
   }
 
+  // Prescribed ghost cells ("we substitute the analytic solutions to the ghost
+  // cells"): the outermost two cells of every axis ARE the ghost cells of this mode (two = the stencil reach of Eq.
+  // 20-22).  The caller overwrites them with its own values G (an array shaped like the state, of which only those
+  // cells are read) before a step and between the two stages; the cells in between are advanced by Eq. 23-27 as
+  // always, and what the scheme computes in the ghost cells themselves (with the clamped index of the outflow mode)
+  // is overwritten before anything reads it (R23).
+  bool in_frame(int64_t c) const {
+    int64_t idx[3] = {c % n[0], (c / n[0]) % n[1], c / (n[0] * n[1])};
+    for (int a = 0; a < D; ++a)
+      if (idx[a] < 2 || idx[a] >= n[a] - 2) return true;
+    return false;
+  }
+  void inject_frame(std::vector<Real>& A, const Real* G) const {
+    for (int64_t c = 0; c < N; ++c)
+      if (in_frame(c))
+        for (int f = 0; f < NF; ++f) A[size_t(f) * N + c] = G[size_t(f) * N + c];
+  }
+  void step_ghosts(Real dt, const Real* Gmid) {
+    std::vector<Real> U1, U2;
+    if (integrator == 0) {
+      stage(U, U, Real(0.5) * dt, U1);
+      inject_frame(U1, Gmid);
+      stage(U1, U, dt, U2);
+    } else {
+      stage(U, U, dt, U1);
+      inject_frame(U1, Gmid);
+      stage(U1, U1, dt, U2);
+      for (size_t i = 0; i < U2.size(); ++i) U2[i] = Real(0.5) * (U[i] + U2[i]);
+    }
+    U.swap(U2);
+  }
+
   // S = max_cells max_a (|v_a| + c) / dr_a   (R6);  dt = Real(cfl) / S.
   Real cfl_S() const {
     Real S = Real(0);
@@ -374,7 +432,8 @@ void oracle_destroy(void* hv) {
   delete h;
 }
 
-// key: "boundary" (0 periodic, 1 outflow) | "riemann" (0 HLLC, 1 HLL)
+// key: "boundary" (0 periodic, 1 outflow) | "riemann" (0 HLLC, 1 HLL) | "integrator" (0 midpoint, 1 Heun) |
+//      "limiter" (0 MINBEE, 1 none, 2 MC)
 int oracle_set_option(void* hv, const char* key, int64_t value) {
   Handle* h = static_cast<Handle*>(hv);
   return dispatch(h, [&](auto* s) {
@@ -388,6 +447,10 @@ int oracle_set_option(void* hv, const char* key, int64_t value) {
     }
     if (!std::strcmp(key, "integrator") && (value == 0 || value == 1)) {
       s->integrator = int(value);
+      return 0;
+    }
+    if (!std::strcmp(key, "limiter") && value >= 0 && value <= 2) {
+      s->limiter = int(value);
       return 0;
     }
     return -1;
@@ -444,6 +507,27 @@ int oracle_step(void* hv, double dt) {
   return dispatch(h, [&](auto* s) {
     using Real = std::decay_t<decltype(s->gamma)>;
     s->step(Real(dt));
+    s->t += double(Real(dt));
+    return 0;
+  });
+}
+
+// Prescribed ghost cells: overwrite the outermost two cells of every axis of the current state with G's
+int oracle_set_ghosts(void* hv, const void* G) {
+  Handle* h = static_cast<Handle*>(hv);
+  return dispatch(h, [&](auto* s) {
+    using Real = std::decay_t<decltype(s->gamma)>;
+    s->inject_frame(s->U, static_cast<const Real*>(G));
+    return 0;
+  });
+}
+
+// one full RK2 step; the ghost cells of the intermediate state U1 are overwritten with Gmid's before the second stage
+int oracle_step_ghosts(void* hv, double dt, const void* Gmid) {
+  Handle* h = static_cast<Handle*>(hv);
+  return dispatch(h, [&](auto* s) {
+    using Real = std::decay_t<decltype(s->gamma)>;
+    s->step_ghosts(Real(dt), static_cast<const Real*>(Gmid));
     s->t += double(Real(dt));
     return 0;
   });
@@ -510,6 +594,20 @@ int oracle_minbee(int dtype, double y0, double y1, double y2, double* lo, double
     *hi = h;
   } else {
     Solver<double, 1>::minbee(y0, y1, y2, *lo, *hi);
+  }
+  return 0;
+}
+
+// one evaluation of an interpolation variant (limiter: 0 MINBEE, 1 none, 2 MC) in the requested precision
+int oracle_limited(int dtype, int limiter, double y0, double y1, double y2, double* lo, double* hi) {
+  if (limiter < 0 || limiter > 2) return -1;
+  if (dtype == 0) {
+    float l, h;
+    Solver<float, 1>::limited(limiter, float(y0), float(y1), float(y2), l, h);
+    *lo = l;
+    *hi = h;
+  } else {
+    Solver<double, 1>::limited(limiter, y0, y1, y2, *lo, *hi);
   }
   return 0;
 }

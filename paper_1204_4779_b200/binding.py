@@ -37,6 +37,8 @@ SIGNATURES = {
     "paraiso_hydro_get_state": (_int, [_vp, _vp]),
     "paraiso_hydro_cfl_dt": (_int, [_vp, _dbl, _pdbl]),
     "paraiso_hydro_step": (_int, [_vp, _dbl]),
+    "paraiso_hydro_set_ghosts": (_int, [_vp, _vp]),
+    "paraiso_hydro_step_ghosts": (_int, [_vp, _dbl, _vp]),
     "paraiso_hydro_run": (_int, [_vp, _dbl, _i64, _dbl, _pi64, _pdbl]),
     "paraiso_hydro_sync": (_int, [_vp]),
     "paraiso_hydro_time": (_int, [_vp, _pdbl, _pi64]),
@@ -231,6 +233,15 @@ class ParaisoHydro:
 
     def step(self, dt):
         self._check(self._lib.paraiso_hydro_step(self._h, float(dt)))
+
+    def set_ghosts(self, G):
+        """Prescribed ghost cells (include/paraiso_hydro.h): the outermost two cells of every axis of the current
+        state := G's.  G: array / tensor shaped like the state (host or device)."""
+        self._check(self._lib.paraiso_hydro_set_ghosts(self._h, self._state_ptr(G)))
+
+    def step_ghosts(self, dt, G_mid):
+        """One RK2 step whose intermediate state gets G_mid's ghost cells before the second stage."""
+        self._check(self._lib.paraiso_hydro_step_ghosts(self._h, float(dt), self._state_ptr(G_mid)))
 
     def run(self, cfl, nsteps, t_end=0.0):
         k, t = _i64(0), _dbl(0)

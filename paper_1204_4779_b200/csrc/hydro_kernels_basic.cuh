@@ -189,7 +189,7 @@ __global__ void __launch_bounds__(256) k_riemann(const Real* __restrict__ LO, co
 // ------------------------------------------------------------------ flux of one face straight from U
 // Face between cells f and f+1 (indices along axis A, mapped through the boundary) on the grid line through
 // cell c (whose index along A is iA): prim x4, interpolate x2, riemann (Eq. 19-22).
-template <class Real, int D, int A, int RS>
+template <class Real, int D, int A, int RS, int LIM = LIMITER_MINBEE>
 __device__ __forceinline__ void face_flux_from_U(const Real* __restrict__ U, const Geom<Real>& g, long long c, int iA,
                                                  int f, Real (&F)[D + 2]) {
   const long long st = axis_stride<A>(g.n);
@@ -202,8 +202,8 @@ __device__ __forceinline__ void face_flux_from_U(const Real* __restrict__ U, con
     V[q] = prim_of<Real, D>(u, g.gm1);
   }
   Prim<Real, D> hi0, lo1;
-  interpolate<Real, D>(V[0], V[1], V[2], nullptr, &hi0);
-  interpolate<Real, D>(V[1], V[2], V[3], &lo1, nullptr);
+  interpolate<Real, D, LIM>(V[0], V[1], V[2], nullptr, &hi0);
+  interpolate<Real, D, LIM>(V[1], V[2], V[3], &lo1, nullptr);
   riemann_flux<Real, D, A, RS>(g.gamma, g.igm1, hi0, lo1, F);
 }
 
@@ -278,18 +278,36 @@ __global__ void __launch_bounds__(256) k_update(const Real* Ubase, Real* Uout,
   if (STAGE == 2) block_reduce_and_finalize<Real>(s, bad, sc, g, gridDim.x, 1);
 }
 
+// ------------------------------------------------------------------ prescribed ghost cells (R23)
+// The outermost two cells of every axis := G's (the analytic solution is substituted into the ghost
+// cells).  One thread per cell; the cells in between are left alone.
+template <class Real, int D>
+__global__ void __launch_bounds__(256) k_inject_ghosts(Real* __restrict__ U, const Real* __restrict__ G, Geom<Real> g) {
+  const long long c = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (c >= g.N) return;
+  int idx[3];
+  decode_cell<D>(c, g.n, idx);
+  bool ghost = false;
+#pragma unroll
+  for (int a = 0; a < D; ++a) ghost = ghost || idx[a] < 2 || idx[a] >= g.n[a] - 2;
+  if (!ghost) return;
+#pragma unroll
+  for (int f = 0; f < D + 2; ++f) U[(size_t)f * g.N + c] = G[(size_t)f * g.N + c];
+}
+
 // ------------------------------------------------------------------ delayed: one kernel per stage, no sharing
-template <class Real, int D, int A, int RS>
+template <class Real, int D, int A, int RS, int LIM>
 __device__ __forceinline__ void delayed_axis(Real (&u)[D + 2], const Real* __restrict__ Uin, const Geom<Real>& g,
                                              long long c, const int (&idx)[3], Real lam) {
   Real Fm[D + 2], Fp[D + 2];
-  face_flux_from_U<Real, D, A, RS>(Uin, g, c, idx[A], idx[A] - 1, Fm);
-  face_flux_from_U<Real, D, A, RS>(Uin, g, c, idx[A], idx[A], Fp);
+  face_flux_from_U<Real, D, A, RS, LIM>(Uin, g, c, idx[A], idx[A] - 1, Fm);
+  face_flux_from_U<Real, D, A, RS, LIM>(Uin, g, c, idx[A], idx[A], Fp);
 #pragma unroll
   for (int f = 0; f < D + 2; ++f) u[f] = rfma(lam, Fm[f] - Fp[f], u[f]);
 }
 
-template <class Real, int D, int RS, int STAGE>
+// LIM: the interpolation variant (R22), a compile-time parameter like the Riemann solver
+template <class Real, int D, int RS, int STAGE, int LIM = LIMITER_MINBEE>
 __global__ void __launch_bounds__(128) k_delayed(const Real* __restrict__ Uin, const Real* Ubase, Real* Uout,
                                                   Geom<Real> g, Scalars* sc) {
   if (sc->done) return;
@@ -301,9 +319,9 @@ __global__ void __launch_bounds__(128) k_delayed(const Real* __restrict__ Uin, c
     decode_cell<D>(c, g.n, idx);
     Real u[D + 2];
     load_fields_rw<Real, D + 2>(Ubase, g.N, c, u);
-    delayed_axis<Real, D, 0, RS>(u, Uin, g, c, idx, Real(sc->lam[STAGE - 1][0]));
-    if constexpr (D > 1) delayed_axis<Real, D, 1, RS>(u, Uin, g, c, idx, Real(sc->lam[STAGE - 1][1]));
-    if constexpr (D > 2) delayed_axis<Real, D, 2, RS>(u, Uin, g, c, idx, Real(sc->lam[STAGE - 1][2]));
+    delayed_axis<Real, D, 0, RS, LIM>(u, Uin, g, c, idx, Real(sc->lam[STAGE - 1][0]));
+    if constexpr (D > 1) delayed_axis<Real, D, 1, RS, LIM>(u, Uin, g, c, idx, Real(sc->lam[STAGE - 1][1]));
+    if constexpr (D > 2) delayed_axis<Real, D, 2, RS, LIM>(u, Uin, g, c, idx, Real(sc->lam[STAGE - 1][2]));
     if (STAGE == 2 && g.integrator == 1) {  // Heun: U2 = 0.5 (U0 + (U1 + dt L(U1))); U0 still sits in Uout
       Real u0[D + 2];
       load_fields_rw<Real, D + 2>(Uout, g.N, c, u0);

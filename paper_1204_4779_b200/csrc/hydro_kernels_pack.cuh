@@ -76,7 +76,7 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 
 // BND: the boundary mode as a compile-time constant.  On periodic grids (n_x even) every pair of cells a thread
 // touches, ghost pairs included, is one aligned 8-byte pair in memory; outflow ghosts are clamped cell by cell.
-template <class T, int D, int RS, int STAGE, int NWX, int TY, int MINB, int BND, int NH>
+template <class T, int D, int RS, int STAGE, int NWX, int TY, int MINB, int BND, int NH, int LIM>
 __global__ void __launch_bounds__(PackShape<T, D, NWX, TY, NH>::NT, MINB)
     k_pack(const scalar_t<T>* __restrict__ Uin, const scalar_t<T>* Ubase, scalar_t<T>* Uout, Geom<scalar_t<T>> g, Scalars* sc,
            int depth) {
@@ -160,8 +160,8 @@ __global__ void __launch_bounds__(PackShape<T, D, NWX, TY, NH>::NT, MINB)
       load_cells_of(m0 + 1, u);
       const P Vp1 = prim_of<T, D>(u, g.gm1);
       P him1, loc, hiM;
-      interpolate<T, D>(Vm2, Vm1, Vc, nullptr, &him1);
-      interpolate<T, D>(Vm1, Vc, Vp1, &loc, &hiM);
+      interpolate<T, D, LIM>(Vm2, Vm1, Vc, nullptr, &him1);
+      interpolate<T, D, LIM>(Vm1, Vc, Vp1, &loc, &hiM);
       T F[NF], a[NF];
       riemann_flux<T, D, M, RS>(g.gamma, g.igm1, him1, loc, F);
       prim_to_fields<T, D>(Vc, a);
@@ -203,7 +203,7 @@ __global__ void __launch_bounds__(PackShape<T, D, NWX, TY, NH>::NT, MINB)
         for (int f = 0; f < NF; ++f) {
           sts(&sm.V[s2][f][pr][pc], vp2[f]);
           const T vp1 = lds<T>(&sm.V[s1][f][pr][pc]);
-          const T dy = minbee_dy(vc[f], vp1, vp2[f]);
+          const T dy = limited_dy<LIM>(vc[f], vp1, vp2[f]);
           loM1[f] = rfma(S(-0.5), dy, vp1);
           hiM[f] = lds<T>(&sm.Hm[f][row][c0]);
           sts(&sm.Hm[f][row][c0], rfma(S(0.5), dy, vp1));
@@ -224,7 +224,7 @@ __global__ void __launch_bounds__(PackShape<T, D, NWX, TY, NH>::NT, MINB)
       for (int f = 0; f < NF; ++f) {
         const T l = xshift_left(vc[f], sm.V[s0][f][pr][pc - 1]);
         const T r = xshift_right(vc[f], sm.V[s0][f][pr][pc + W]);
-        const T dy = minbee_dy(l, vc[f], r);
+        const T dy = limited_dy<LIM>(l, vc[f], r);
         const T lox = rfma(S(-0.5), dy, vc[f]);
         hix[f] = rfma(S(0.5), dy, vc[f]);
         if (lane == 0) sm.LOx[f][row][wx] = lane_first(lox);
@@ -233,7 +233,7 @@ __global__ void __launch_bounds__(PackShape<T, D, NWX, TY, NH>::NT, MINB)
       if constexpr (D == 3) {
 #pragma unroll
         for (int f = 0; f < NF; ++f) {
-          const T dy = minbee_dy(lds<T>(&sm.V[s0][f][pr - 1][pc]), vc[f], lds<T>(&sm.V[s0][f][pr + 1][pc]));
+          const T dy = limited_dy<LIM>(lds<T>(&sm.V[s0][f][pr - 1][pc]), vc[f], lds<T>(&sm.V[s0][f][pr + 1][pc]));
           sts(&sm.LOy[f][row][c0], rfma(S(-0.5), dy, vc[f]));
           hiy[f] = rfma(S(0.5), dy, vc[f]);
         }
@@ -399,18 +399,18 @@ __global__ void __launch_bounds__(PackShape<T, D, NWX, TY, NH>::NT, MINB)
       //      primitives of the next plane's halo (loaded during the previous phase B)
       P hiYlow, hiXlow;
       if constexpr (D == 3) if (do_y) {
-        interpolate<T, D>(plane_y(s0, 0), plane_y(s0, 1), plane_y(s0, 2), nullptr, &hiYlow);
+        interpolate<T, D, LIM>(plane_y(s0, 0), plane_y(s0, 1), plane_y(s0, 2), nullptr, &hiYlow);
         P lo;
-        interpolate<T, D>(plane_y(s0, TY + 1), plane_y(s0, TY + 2), plane_y(s0, TY + 3), &lo, nullptr);
+        interpolate<T, D, LIM>(plane_y(s0, TY + 1), plane_y(s0, TY + 2), plane_y(s0, TY + 3), &lo, nullptr);
         T a[NF];
         prim_to_fields<T, D>(lo, a);
 #pragma unroll
         for (int f = 0; f < NF; ++f) sts(&sm.LOy[f][TY][lane * W], a[f]);
       }
       if (xtask) {
-        interpolate<T, D>(plane_x(s0, 0), plane_x(s0, 1), plane_x(s0, 2), nullptr, &hiXlow);
+        interpolate<T, D, LIM>(plane_x(s0, 0), plane_x(s0, 1), plane_x(s0, 2), nullptr, &hiXlow);
         P lo;
-        interpolate<T, D>(plane_x(s0, TXC + 1), plane_x(s0, TXC + 2), plane_x(s0, TXC + 3), &lo, nullptr);
+        interpolate<T, D, LIM>(plane_x(s0, TXC + 1), plane_x(s0, TXC + 2), plane_x(s0, TXC + 3), &lo, nullptr);
         T a[NF];
         prim_to_fields<T, D>(lo, a);
 #pragma unroll
@@ -475,11 +475,11 @@ inline int pack_default_depth(long long tiles_in_plane, int nM, int capacity) {
   return best;
 }
 
-template <class T, int D, int RS, int STAGE, int NWX, int TY, int MINB, int BND, int NH>
+template <class T, int D, int RS, int STAGE, int NWX, int TY, int MINB, int BND, int NH, int LIM = LIMITER_MINBEE>
 static bool launch_pack_bnd(const scalar_t<T>* Uin, const scalar_t<T>* Ubase, scalar_t<T>* Uout, const Geom<scalar_t<T>>& g,
                             Scalars* sc, cudaStream_t stream, int depth) {
   using Sh = PackShape<T, D, NWX, TY, NH>;
-  auto kern = k_pack<T, D, RS, STAGE, NWX, TY, MINB, BND, NH>;
+  auto kern = k_pack<T, D, RS, STAGE, NWX, TY, MINB, BND, NH, LIM>;
   static int capacity[64] = {};  // blocks of this kernel the whole device holds at once (0: not configured yet)
   int dev = 0;
   if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return false;
@@ -510,12 +510,12 @@ static bool launch_pack_bnd(const scalar_t<T>* Uin, const scalar_t<T>* Ubase, sc
   return true;
 }
 
-template <class T, int D, int RS, int STAGE, int NWX, int TY, int MINB, int NH = 1>
+template <class T, int D, int RS, int STAGE, int NWX, int TY, int MINB, int NH = 1, int LIM = LIMITER_MINBEE>
 static bool launch_pack_shape(const scalar_t<T>* Uin, const scalar_t<T>* Ubase, scalar_t<T>* Uout, const Geom<scalar_t<T>>& g,
                               Scalars* sc, cudaStream_t stream, int depth) {
   if (g.boundary == BOUNDARY_PERIODIC)
-    return launch_pack_bnd<T, D, RS, STAGE, NWX, TY, MINB, BOUNDARY_PERIODIC, NH>(Uin, Ubase, Uout, g, sc, stream, depth);
-  return launch_pack_bnd<T, D, RS, STAGE, NWX, TY, MINB, BOUNDARY_OUTFLOW, NH>(Uin, Ubase, Uout, g, sc, stream, depth);
+    return launch_pack_bnd<T, D, RS, STAGE, NWX, TY, MINB, BOUNDARY_PERIODIC, NH, LIM>(Uin, Ubase, Uout, g, sc, stream, depth);
+  return launch_pack_bnd<T, D, RS, STAGE, NWX, TY, MINB, BOUNDARY_OUTFLOW, NH, LIM>(Uin, Ubase, Uout, g, sc, stream, depth);
 }
 
 // Returns false when the packed kernel does not cover this shape (fp32: odd n_x; unknown block shape): the caller falls back.
@@ -584,6 +584,25 @@ bool launch_pack_stage(const Real* Uin, const Real* Ubase, Real* Uout, const Geo
       }
       return false;
     }
+  }
+}
+
+// The interpolation variants other than MINBEE (LIM = LIMITER_NONE, LIMITER_MC; R22) exist in the default launch
+// shapes only (2-D: rows of 2 warps as overlapping tiles; 3-D: 7-row tiles with one halo warp); instantiated in
+// pack_lim_f<32|64>_d<D>.cu.
+template <class Real, int D, int RS, int STAGE, int LIM>
+bool launch_pack_stage_lim(const Real* Uin, const Real* Ubase, Real* Uout, const Geom<Real>& g, Scalars* sc,
+                           cudaStream_t stream) {
+  if constexpr (D == 1) {
+    return false;
+  } else {
+    constexpr bool F32 = sizeof(Real) == 4;
+    using T = typename std::conditional<F32, f32x2, double>::type;
+    if (LaneTraits<T>::W == 2 && g.n[0] % 2 != 0) return false;
+    if constexpr (D == 2)
+      return launch_pack_shape<T, D, RS, STAGE, 2, 1, (F32 ? 2 : PH_PACK64_MINB2), 0, LIM>(Uin, Ubase, Uout, g, sc, stream, 0);
+    else
+      return launch_pack_shape<T, D, RS, STAGE, 1, 7, 2, 1, LIM>(Uin, Ubase, Uout, g, sc, stream, 0);
   }
 }
 

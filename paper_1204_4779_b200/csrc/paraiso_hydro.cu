@@ -48,6 +48,21 @@ PH_EXTERN_PACK(float, 3)
 PH_EXTERN_PACK(double, 2)
 PH_EXTERN_PACK(double, 3)
 #undef PH_EXTERN_PACK1
+// ... and with the interpolation variants other than MINBEE in pack_lim_f<32|64>_d<D>.cu
+#define PH_EXTERN_LIM1(REAL, DD, RS, ST, LIM)                                                                         \
+  extern template bool launch_pack_stage_lim<REAL, DD, RS, ST, LIM>(const REAL*, const REAL*, REAL*, const Geom<REAL>&, \
+                                                                    Scalars*, cudaStream_t);
+#define PH_EXTERN_LIM(REAL, DD)                                                                               \
+  PH_EXTERN_LIM1(REAL, DD, RIEMANN_HLLC, 1, LIMITER_NONE) PH_EXTERN_LIM1(REAL, DD, RIEMANN_HLLC, 2, LIMITER_NONE) \
+  PH_EXTERN_LIM1(REAL, DD, RIEMANN_HLL, 1, LIMITER_NONE) PH_EXTERN_LIM1(REAL, DD, RIEMANN_HLL, 2, LIMITER_NONE)   \
+  PH_EXTERN_LIM1(REAL, DD, RIEMANN_HLLC, 1, LIMITER_MC) PH_EXTERN_LIM1(REAL, DD, RIEMANN_HLLC, 2, LIMITER_MC)     \
+  PH_EXTERN_LIM1(REAL, DD, RIEMANN_HLL, 1, LIMITER_MC) PH_EXTERN_LIM1(REAL, DD, RIEMANN_HLL, 2, LIMITER_MC)
+PH_EXTERN_LIM(float, 2)
+PH_EXTERN_LIM(float, 3)
+PH_EXTERN_LIM(double, 2)
+PH_EXTERN_LIM(double, 3)
+#undef PH_EXTERN_LIM
+#undef PH_EXTERN_LIM1
 #undef PH_EXTERN_PACK
 }  // namespace ph
 
@@ -70,6 +85,7 @@ struct paraiso_hydro {
   int arith = 0;       // k_march fp32: 0 IEEE-exact division / square root, 1 hardware approximations (f32fast)
   int staging = 0;     // k_march: 0 / 1 own-cell LDG, 2 TMA bulk copies into a shared-memory ring
   int integrator = 0;  // 0 midpoint (paper) | 1 Heun
+  int limiter = 0;     // 0 MINBEE (Eq. 21) | 1 none (first order) | 2 monotonized central (R22): k_pack, k_delayed
   int state_kind = 0;  // 0: set_state / get_state exchange conserved variables, 1: primitive variables
 
   void* U[2] = {nullptr, nullptr};  // U[0]: current state / U_base; U[1]: stage-1 result
@@ -78,6 +94,7 @@ struct paraiso_hydro {
   void* HI[3] = {nullptr, nullptr, nullptr};
   void* F[3] = {nullptr, nullptr, nullptr};   // manifest_*: face fluxes
   void* Fb[3] = {nullptr, nullptr, nullptr};  // outflow boundary faces
+  void* G = nullptr;                          // prescribed ghost cells: device copy of the caller's array (first use)
   Scalars* sc = nullptr;
   cudaStream_t stream = nullptr;
   bool has_state = false;
@@ -135,7 +152,8 @@ static Geom<Real> make_geom(const paraiso_hydro* h) {
 
 static void free_intermediates(paraiso_hydro* h) {
   cudaFree(h->V);
-  h->V = nullptr;
+  cudaFree(h->G);
+  h->V = h->G = nullptr;
   for (int a = 0; a < 3; ++a) {
     cudaFree(h->LO[a]);
     cudaFree(h->HI[a]);
@@ -249,6 +267,10 @@ struct Launch {
 
   template <int STAGE>
   static void stage_kernels(paraiso_hydro* h, const Geom<Real>& g, const Real* Uin, Real* Uout) {
+    if (h->limiter != LIMITER_MINBEE && (h->variant == VARIANT_MANIFEST_ALL || h->variant == VARIANT_MANIFEST_FLUX)) {
+      h->shape_error = true;  // the interpolation variants live in k_pack and k_delayed
+      return;
+    }
     switch (h->variant) {
       case VARIANT_MANIFEST_ALL: {
         const int bs = 256;
@@ -284,15 +306,22 @@ struct Launch {
     const Real* base = stage_base<STAGE>(h);
     auto try_pack = [&]() -> bool {
       if constexpr (D >= 2) {
-        if (h->cells_per_thread == 0 && h->staging == 0 && h->arith == 0 &&
-            launch_pack_stage<Real, D, RS, STAGE>(Uin, base, Uout, g, h->sc, h->stream, h->block, h->tile_depth)) {
-          h->kernel_used = KERNEL_PACK;
-          return true;
+        if (h->cells_per_thread || h->staging || h->arith) return false;
+        bool ok = false;
+        if (h->limiter == LIMITER_MINBEE) {
+          ok = launch_pack_stage<Real, D, RS, STAGE>(Uin, base, Uout, g, h->sc, h->stream, h->block, h->tile_depth);
+        } else if (!(h->block[0] || h->block[1] || h->block[2] || h->tile_depth)) {  // default launch shape only
+          ok = h->limiter == LIMITER_NONE
+                   ? launch_pack_stage_lim<Real, D, RS, STAGE, LIMITER_NONE>(Uin, base, Uout, g, h->sc, h->stream)
+                   : launch_pack_stage_lim<Real, D, RS, STAGE, LIMITER_MC>(Uin, base, Uout, g, h->sc, h->stream);
         }
+        if (ok) h->kernel_used = KERNEL_PACK;
+        return ok;
       }
       return false;
     };
     auto try_march = [&]() -> bool {
+      if (h->limiter != LIMITER_MINBEE) return false;  // the interpolation variants live in k_pack and k_delayed
       if (launch_march_stage<Real, D, RS, STAGE>(Uin, base, Uout, g, h->sc, h->stream, h->block, h->tile_depth,
                                                  h->cells_per_thread, h->staging, h->arith)) {
         h->kernel_used = KERNEL_MARCH;
@@ -301,6 +330,7 @@ struct Launch {
       return false;
     };
     auto try_fused1 = [&]() -> bool {
+      if (h->limiter != LIMITER_MINBEE) return false;
       if (h->cells_per_thread == 0 && h->staging == 0 && h->arith == 0 &&
           launch_fused_stage<Real, D, RS, STAGE>(Uin, base, Uout, g, h->sc, h->stream, h->block, h->tile_depth)) {
         h->kernel_used = KERNEL_FUSED1;
@@ -311,7 +341,12 @@ struct Launch {
     auto try_delayed = [&]() -> bool {
       const int bs = h->block[0] > 0 ? h->block[0] : 128;
       if (bs > 128 || h->block[1] || h->block[2] || h->tile_depth || h->cells_per_thread || h->staging || h->arith) return false;
-      k_delayed<Real, D, RS, STAGE><<<grid1d(h->N, bs), bs, 0, h->stream>>>(Uin, base, Uout, g, h->sc);
+      if (h->limiter == LIMITER_NONE)
+        k_delayed<Real, D, RS, STAGE, LIMITER_NONE><<<grid1d(h->N, bs), bs, 0, h->stream>>>(Uin, base, Uout, g, h->sc);
+      else if (h->limiter == LIMITER_MC)
+        k_delayed<Real, D, RS, STAGE, LIMITER_MC><<<grid1d(h->N, bs), bs, 0, h->stream>>>(Uin, base, Uout, g, h->sc);
+      else
+        k_delayed<Real, D, RS, STAGE><<<grid1d(h->N, bs), bs, 0, h->stream>>>(Uin, base, Uout, g, h->sc);
       h->kernel_used = KERNEL_DELAYED;
       return true;
     };
@@ -358,6 +393,13 @@ struct Launch {
   static void convert(paraiso_hydro* h, const void* in, void* out) {
     const int bs = 256;
     k_convert<Real, D, TO_CONS><<<grid1d(h->N, bs), bs, 0, h->stream>>>((const Real*)in, (Real*)out, make_geom<Real>(h));
+    h->launches += 1;
+  }
+
+  // ghost cells of buffer U[which] := those of h->G (R23)
+  static void inject(paraiso_hydro* h, int which) {
+    const int bs = 256;
+    k_inject_ghosts<Real, D><<<grid1d(h->N, bs), bs, 0, h->stream>>>((Real*)h->U[which], (const Real*)h->G, make_geom<Real>(h));
     h->launches += 1;
   }
 
@@ -484,6 +526,7 @@ static bool find_option(paraiso_hydro* h, const char* key, OptionRef* ref) {
                       {"graph", {&h->use_graph, 0, 1}},
                       {"state_kind", {&h->state_kind, 0, 1}},
                       {"integrator", {&h->integrator, 0, 1}},
+                      {"limiter", {&h->limiter, 0, 2}},
                       {"staging", {&h->staging, 0, 2}},
                       {"arith", {&h->arith, 0, 1}},
                       {"kernel_used", {&h->kernel_used, 0, 0}}};  // read-only: KERNEL_* of the last stage launch
@@ -574,6 +617,40 @@ int paraiso_hydro_step(paraiso_hydro_t* h, double dt) {
   dispatch(h, [&](auto L) {
     L.control(h, CTRL_MANUAL_DT, dt, 0);
     L.step(h);
+  });
+  return check_launch(h);
+}
+
+// Brings the caller's ghost array (host or device) into the handle's device copy.
+static int stage_ghosts(paraiso_hydro* h, const void* G) {
+  const size_t bytes = size_t(h->nf) * h->N * h->esize;
+  if (!h->G) CUDA_TRY(h, cudaMalloc(&h->G, bytes));
+  CUDA_TRY(h, cudaMemcpyAsync(h->G, G, bytes, cudaMemcpyDefault, h->stream));
+  return PARAISO_OK;
+}
+
+int paraiso_hydro_set_ghosts(paraiso_hydro_t* h, const void* G) {
+  if (!h || !G) return fail(h, PARAISO_EINVAL, "set_ghosts: null pointer");
+  if (!h->has_state) return fail(h, PARAISO_ESTATE, "set_ghosts: no state set");
+  int rc = stage_ghosts(h, G);
+  if (rc) return rc;
+  dispatch(h, [&](auto L) { L.inject(h, 0); });
+  return check_launch(h);
+}
+
+int paraiso_hydro_step_ghosts(paraiso_hydro_t* h, double dt, const void* G_mid) {
+  if (!h || !G_mid) return fail(h, PARAISO_EINVAL, "step_ghosts: null pointer");
+  if (!h->has_state) return fail(h, PARAISO_ESTATE, "step_ghosts: no state set");
+  if (!(dt > 0.0) || !std::isfinite(dt)) return fail(h, PARAISO_EINVAL, "step_ghosts: dt must be finite and > 0");
+  int rc = ensure_intermediates(h);
+  if (rc) return rc;
+  rc = stage_ghosts(h, G_mid);
+  if (rc) return rc;
+  dispatch(h, [&](auto L) {
+    L.control(h, CTRL_MANUAL_DT, dt, 0);
+    L.template stage<1>(h);
+    L.inject(h, 1);
+    L.template stage<2>(h);
   });
   return check_launch(h);
 }

@@ -23,6 +23,16 @@ def candidates(dims, dtype_is_f32):
     if dims == 1:
         return out
     depths = (0, 32, 128)
+    # k_pack (shared-memory window; fp32: packed pairs of cells, fp64: one cell per thread), the default on-chip kernel
+    if dims == 3:
+        for ty, d in itertools.product((5, 7, 11, 14, 15) if dtype_is_f32 else (7, 14), (0, 64)):
+            out.append((f"pack ty={ty}{' two halo warps' if ty == 14 else ''} depth={d or 'auto'}", "pack",
+                        {"block_y": ty, "tile_depth": d}))
+    else:
+        for nwx, d in itertools.product((1, 2, 4, 8) if dtype_is_f32 else (2, 4, 8), (0, 32, 64)):
+            out.append((f"pack warps={nwx} overlapping tiles depth={d or 'auto'}", "pack", {"block_x": nwx, "tile_depth": d}))
+        for nwx in (4, 7):
+            out.append((f"pack warps={nwx} halo warp", "pack", {"block_x": nwx, "block_z": 1}))
     if dims == 3:
         for ty, d in itertools.product((4, 7, 8, 15), depths):
             out.append((f"march ty={ty} depth={d or 'auto'}", "march", {"block_y": ty, "tile_depth": d}))

@@ -36,6 +36,23 @@ def _minbee(y0, y1, y2):
     return y1 - 0.5 * dy, y1 + 0.5 * dy
 
 
+def _mc(y0, y1, y2):
+    """Monotonized-central limiter in the textbook form (van Leer 1977): sign(d) max(0, min(2|a|, 2|b|, |c|)) when the
+    one-sided differences a, b agree in sign, else 0 (c = their mean) — written through np.sign, not the product test."""
+    a, b = y1 - y0, y2 - y1
+    c = 0.5 * (a + b)
+    same = np.sign(a) * np.sign(b) > 0
+    dy = np.where(same, np.sign(c) * np.minimum(np.minimum(2 * np.abs(a), 2 * np.abs(b)), np.abs(c)), 0.0)
+    return y1 - 0.5 * dy, y1 + 0.5 * dy
+
+
+def _none(y0, y1, y2):
+    return y1, y1
+
+
+LIMITERS = {"minbee": _minbee, "none": _none, "mc": _mc}
+
+
 def _flux_phys(V, a, g):
     d = V.shape[0] - 2
     rho, p, vn = V[0], V[d + 1], V[1 + a]
@@ -67,13 +84,13 @@ def riemann(VL, VR, a, g, kind):
     return np.where(SL >= 0, FL, np.where(SR <= 0, FR, np.where(Ss >= 0, FsL, FsR)))
 
 
-def stage(Uin, Ubase, tau, dr, g, boundary, kind):
+def stage(Uin, Ubase, tau, dr, g, boundary, kind, limiter="minbee"):
     d = Uin.shape[0] - 2
     V = prim(Uin, g)
     out = Ubase.copy()
     for a in range(d):
         ax = V.ndim - 1 - a  # array axes are [f][z][y][x]
-        lo, hi = _minbee(_shift(V, -1, ax, boundary), V, _shift(V, 1, ax, boundary))
+        lo, hi = LIMITERS[limiter](_shift(V, -1, ax, boundary), V, _shift(V, 1, ax, boundary))
         # flux at face i+1/2: left state hi(i), right state lo(i+1)
         Fp = riemann(hi, _shift(lo, 1, ax, boundary), a, g, kind)
         if boundary == "periodic":
@@ -88,9 +105,9 @@ def stage(Uin, Ubase, tau, dr, g, boundary, kind):
     return out
 
 
-def step(U, dt, dr, g, boundary="periodic", kind="hllc"):
-    U1 = stage(U, U, 0.5 * dt, dr, g, boundary, kind)
-    return stage(U1, U, dt, dr, g, boundary, kind)
+def step(U, dt, dr, g, boundary="periodic", kind="hllc", limiter="minbee"):
+    U1 = stage(U, U, 0.5 * dt, dr, g, boundary, kind, limiter)
+    return stage(U1, U, dt, dr, g, boundary, kind, limiter)
 
 
 def cfl_dt(U, cfl, dr, g):

@@ -473,7 +473,101 @@ def test_fast_arithmetic_option_stays_inside_the_tolerances(gpu, oracle_mod, dim
 
 
 def test_fast_arithmetic_option_on_kelvin_helmholtz(gpu, oracle_mod):
+    """arith = 1 on config 1's recipe (256^2), with BOTH error metrics: DESIGN.md R17 (momentum components on their
+    common scale) against north_star's tolerances, and SURVEY A17 read strictly (every field on its OWN max |ref|; the
+    transverse momentum m_y, max ~ 0.02 beside m_x ~ 1, is the tight case).  The strict figure is what DESIGN.md R21
+    quotes: one step is inside 1e-5 on every field except m_y, which the test bounds at 1e-4 (measured 3-4e-5)."""
+    from parity_util import own_scale_errors
+
     w = inputs.kelvin_helmholtz(256, dtype=np.float32, seed=0, steps=100)  # config 1's recipe at 256^2
-    ref, _ = oracle_steps(oracle_mod, w, 100)
-    got, _ = gpu_steps(gpu, w, 100, "march", arith=1)
-    assert np.all(field_errors(got, ref) <= 1e-3), field_errors(got, ref)
+    for nsteps, tol in ((1, 1e-5), (100, 1e-3)):
+        ref, _ = oracle_steps(oracle_mod, w, nsteps)
+        got, _ = gpu_steps(gpu, w, nsteps, "march", arith=1)
+        shared, own = field_errors(got, ref), own_scale_errors(got, ref)
+        print(f"arith=1 KH 256^2 after {nsteps} step(s): R17 metric {shared}, per-field own scale {own}")
+        assert np.all(shared <= tol), shared
+        assert np.all(np.delete(own, 2) <= tol), own          # rho, m_x, E on their own scale: inside the tolerance
+        assert own[2] <= 10 * tol, own                        # m_y on its own scale: reported, bounded a decade above
+
+
+LIMITER_ID = {"minbee": 0, "none": 1, "mc": 2}
+
+
+@pytest.mark.parametrize("limiter", ["none", "mc"])
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("dims", [1, 2, 3])
+def test_limiter_option_matches_oracle(gpu, oracle_mod, dims, dtype, limiter):
+    """Option limiter (R22): no slopes (first-order Godunov) and the monotonized-central
+    limiter as compile-time variants of k_pack (default launch shape) and k_delayed; both Riemann solvers, both
+    boundaries, stepped by hand and device-paced: bit-equal to the oracle run with the same option.  The kernels that do
+    not carry the variants answer PARAISO_EINVAL."""
+    import torch
+
+    n = {1: (517,), 2: (204, 61), 3: (46, 30, 21)}[dims]
+    for boundary, riemann in (("periodic", "hllc"), ("outflow", "hll")):
+        w = inputs.random_smooth(n, dtype, seed=71 + dims, boundary=boundary)
+        o = oracle_mod.Oracle(w.n, w.extent, w.gamma, w.dtype, boundary, riemann, "omp", "midpoint", limiter)
+        o.set_state(w.U)
+        k, t = o.run(w.cfl, 11)
+        ref = o.get_state()
+        o.close()
+        for variant in ("fused", "pack", "delayed"):
+            if variant == "pack" and dims == 1:
+                continue
+            with gpu.ParaisoHydro(w.n, w.extent, w.gamma, w.dtype, boundary, riemann, variant,
+                                  limiter=LIMITER_ID[limiter]) as h:
+                h.set_state(torch.from_numpy(w.U).cuda())
+                for _ in range(2):
+                    h.step(h.cfl_dt(w.cfl))
+                h.run(w.cfl, 9)
+                got = h.get_state()
+                tg, kg = h.time()
+                assert h.stats() == 0 and kg == 11
+                assert h.get_option("kernel_used") == KERNEL_ID["delayed" if (variant == "delayed" or dims == 1) else "pack"]
+            assert abs(tg - t) <= 20 * TOL[np.dtype(dtype)][2] * t
+            assert np.array_equal(got, ref), (variant, boundary, field_errors(got, ref))
+    # the slopes really are off / different: the three variants give three different states
+    w = inputs.random_smooth(n, dtype, seed=71 + dims)
+    states = [gpu_steps(gpu, w, 3, "fused", limiter=i)[0] for i in (0, 1, 2)]
+    assert not np.array_equal(states[0], states[1]) and not np.array_equal(states[0], states[2])
+    if dims > 1:
+        for variant, opts in (("march", {}), ("fused1", {}), ("manifest_flux", {}), ("manifest_all", {}), ("pack", {"tile_depth": 8})):
+            with gpu.ParaisoHydro(w.n, w.extent, w.gamma, w.dtype, "periodic", "hllc", variant, limiter=2, **opts) as h:
+                h.set_state(w.U)
+                with pytest.raises(gpu.ParaisoError) as ei:
+                    h.step(1e-4)
+                assert ei.value.code == gpu.PARAISO_EINVAL
+
+
+@pytest.mark.parametrize("variant", ["fused", "march", "delayed", "manifest_flux"])
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("dims", [1, 2, 3])
+def test_prescribed_ghost_cells_match_oracle(gpu, oracle_mod, dims, dtype, variant):
+    """set_ghosts / step_ghosts (R23): the outermost two cells of every axis are overwritten
+    with the caller's values before each step and between the stages; host and device arrays; bit-equal to the oracle."""
+    import torch
+
+    n = grid_for("pack", {1: (131,), 2: (70, 37), 3: (38, 21, 17)}[dims])
+    if not covers(variant, dims, dtype, n):
+        pytest.skip("kernel does not cover this grid kind")
+    w = inputs.random_smooth(n, dtype, seed=81 + dims, boundary="outflow")
+    rng = np.random.default_rng(7)
+    frames = [np.ascontiguousarray((w.U * (1.0 + 0.03 * rng.uniform(-1, 1, w.U.shape))).astype(dtype)) for _ in range(6)]
+    o = oracle_mod.Oracle(w.n, w.extent, w.gamma, w.dtype, "outflow", "hllc", "omp")
+    o.set_state(w.U)
+    dt = 0.5 * o.cfl_dt(w.cfl)
+    with gpu.ParaisoHydro(w.n, w.extent, w.gamma, w.dtype, "outflow", "hllc", variant) as h:
+        h.set_state(torch.from_numpy(w.U).cuda())
+        for k in range(3):
+            o.set_ghosts(frames[2 * k])
+            o.step_ghosts(dt, frames[2 * k + 1])
+            if k == 1:  # device arrays
+                h.set_ghosts(torch.from_numpy(frames[2 * k]).cuda())
+                h.step_ghosts(dt, torch.from_numpy(frames[2 * k + 1]).cuda())
+            else:       # host arrays
+                h.set_ghosts(frames[2 * k])
+                h.step_ghosts(dt, frames[2 * k + 1])
+        got = h.get_state()
+        assert h.time()[1] == 3
+    assert np.array_equal(got, o.get_state()), field_errors(got, o.get_state())
+    o.close()
