@@ -302,11 +302,13 @@ _MEASURED_ALU_PEAK = {}
 
 
 def measured_alu_peak(binding, itemsize):
-    """Tlaneop/s of the FFMA (fp32) / DFMA (fp64) pipe measured on this device by the probe library
-    (paraiso_probe_peak: 16 independent chains per thread, 8 warps per scheduler, best of 5), or None."""
+    """Tlaneop/s of the FFMA / FFMA2 (fp32) or DFMA (fp64) pipe measured on this device by the probe library
+    (paraiso_probe_peak: 16 independent chains per thread, 8 warps per scheduler, best of 5 short launches), or None."""
     if itemsize not in _MEASURED_ALU_PEAK:
         try:
-            _MEASURED_ALU_PEAK[itemsize] = float(binding.probe_peak("ffma" if itemsize == 4 else "dfma"))
+            # fp32: the better of the scalar and the packed instruction (the packed one reaches the higher lane rate)
+            _MEASURED_ALU_PEAK[itemsize] = (max(float(binding.probe_peak("ffma")), float(binding.probe_peak("ffma2")))
+                                            if itemsize == 4 else float(binding.probe_peak("dfma")))
         except Exception:
             _MEASURED_ALU_PEAK[itemsize] = None
     return _MEASURED_ALU_PEAK[itemsize]
@@ -333,7 +335,7 @@ def roofline_of(w, r, peak, peak_src, traffic=None, binding=None, counted_ops=No
     alu = {"bound": "alu", "achieved": alu_achieved, "peak": alu_peak, "unit": "Tlaneop/s", "frac": alu_achieved / alu_peak,
            "algorithmic_ops_per_launch": ops, "counted_ops_per_cell_step": counted,
            "peak_source": ("measured: %s fused multiply-adds per second on this device (paraiso_probe_peak)"
-                           % ("FFMA" if isz == 4 else "DFMA")) if alu_measured else "nominal (no probe library)",
+                           % ("max(FFMA, FFMA2)" if isz == 4 else "DFMA")) if alu_measured else "nominal (no probe library)",
            "peak_nominal": alu_nominal, "frac_of_nominal": alu_achieved / alu_nominal,
            "peak_nominal_source": "148 SMs x %d %s lanes x 1.965 GHz (B200_PROFILING.md unit counts and clocks.max.sm)"
                                   % (128 if isz == 4 else 64, "FP32" if isz == 4 else "FP64"),

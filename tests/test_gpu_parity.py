@@ -475,8 +475,9 @@ def test_fast_arithmetic_option_stays_inside_the_tolerances(gpu, oracle_mod, dim
 def test_fast_arithmetic_option_on_kelvin_helmholtz(gpu, oracle_mod):
     """arith = 1 on config 1's recipe (256^2), with BOTH error metrics: DESIGN.md R17 (momentum components on their
     common scale) against north_star's tolerances, and SURVEY A17 read strictly (every field on its OWN max |ref|; the
-    transverse momentum m_y, max ~ 0.02 beside m_x ~ 1, is the tight case).  The strict figure is what DESIGN.md R21
-    quotes: one step is inside 1e-5 on every field except m_y, which the test bounds at 1e-4 (measured 3-4e-5)."""
+    transverse momentum m_y, max ~ 0.02 beside m_x ~ 1, is the tight case).  Measured on B200: after one step m_y is
+    8.3e-6 of its own maximum (the other fields 2-3e-7), after 100 steps 1.2e-4 (the others ~2e-6): inside north_star's
+    1e-5 / 1e-3 under either metric, which is what DESIGN.md R21 quotes."""
     from parity_util import own_scale_errors
 
     w = inputs.kelvin_helmholtz(256, dtype=np.float32, seed=0, steps=100)  # config 1's recipe at 256^2
@@ -486,8 +487,7 @@ def test_fast_arithmetic_option_on_kelvin_helmholtz(gpu, oracle_mod):
         shared, own = field_errors(got, ref), own_scale_errors(got, ref)
         print(f"arith=1 KH 256^2 after {nsteps} step(s): R17 metric {shared}, per-field own scale {own}")
         assert np.all(shared <= tol), shared
-        assert np.all(np.delete(own, 2) <= tol), own          # rho, m_x, E on their own scale: inside the tolerance
-        assert own[2] <= 10 * tol, own                        # m_y on its own scale: reported, bounded a decade above
+        assert np.all(own <= tol), own  # every field on its own scale, m_y included
 
 
 LIMITER_ID = {"minbee": 0, "none": 1, "mc": 2}
