@@ -157,3 +157,53 @@ def limited(limiter, y0, y1, y2, dtype=np.float64):
 
 def num_threads(kind="omp"):
     return _lib(kind).oracle_num_threads()
+
+
+class Wave:
+    """The paper's linear-wave example (§2.3, Table 2) as oracle/wave_oracle.cpp states it: fp64, periodic on
+    [0, 2 pi), dx = 2 pi / n, dt = dx / c.  step() advances one step and returns the discrete energy of Eq. 8."""
+
+    def __init__(self, n, c=3.43):
+        L = ctypes.CDLL(_build.build()["wave"])
+        vp, dbl = ctypes.c_void_p, ctypes.c_double
+        L.wave_oracle_create.restype = vp
+        L.wave_oracle_create.argtypes = [ctypes.c_int64, dbl]
+        L.wave_oracle_destroy.argtypes = [vp]
+        L.wave_oracle_destroy.restype = None
+        L.wave_oracle_set_state.argtypes = [vp, vp, vp]
+        L.wave_oracle_get_state.argtypes = [vp, vp, vp]
+        L.wave_oracle_step.argtypes = [vp]
+        L.wave_oracle_step.restype = dbl
+        L.wave_oracle_dx.argtypes = [vp]
+        L.wave_oracle_dx.restype = dbl
+        L.wave_oracle_dt.argtypes = [vp]
+        L.wave_oracle_dt.restype = dbl
+        self._L, self.n = L, int(n)
+        self._h = L.wave_oracle_create(self.n, float(c))
+        if not self._h:
+            raise ValueError("wave_oracle_create failed")
+        self.dx, self.dt = L.wave_oracle_dx(self._h), L.wave_oracle_dt(self._h)
+
+    def set_state(self, f, g):
+        f, g = np.ascontiguousarray(f, np.float64), np.ascontiguousarray(g, np.float64)
+        assert f.shape == g.shape == (self.n,)
+        self._L.wave_oracle_set_state(self._h, f.ctypes.data, g.ctypes.data)
+
+    def get_state(self):
+        f, g = np.empty(self.n), np.empty(self.n)
+        self._L.wave_oracle_get_state(self._h, f.ctypes.data, g.ctypes.data)
+        return f, g
+
+    def step(self):
+        return self._L.wave_oracle_step(self._h)
+
+    def close(self):
+        if self._h:
+            self._L.wave_oracle_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

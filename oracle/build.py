@@ -14,11 +14,12 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "euler_oracle.cpp")
+WAVE_SRC = os.path.join(HERE, "wave_oracle.cpp")  # the paper's linear-wave example (§2.3), a library of its own
 BASE = ["g++", "-O2", "-std=c++17", "-ffp-contract=off", "-mfma", "-shared", "-fPIC", "-Wall", "-Wno-unknown-pragmas"]
 
 
-def _stale(out):
-    return not os.path.exists(out) or os.path.getmtime(out) < os.path.getmtime(SRC)
+def _stale(out, src=SRC):
+    return not os.path.exists(out) or os.path.getmtime(out) < os.path.getmtime(src)
 
 
 def build(force=False, verbose=False):
@@ -31,6 +32,13 @@ def build(force=False, verbose=False):
                 print(" ".join(cmd))
             subprocess.run(cmd, check=True)
         outs[name] = out
+    out = os.path.join(HERE, "liboracle_wave.so")
+    if force or _stale(out, WAVE_SRC):
+        cmd = BASE + [WAVE_SRC, "-o", out]
+        if verbose:
+            print(" ".join(cmd))
+        subprocess.run(cmd, check=True)
+    outs["wave"] = out
     return outs
 
 

@@ -49,6 +49,16 @@ SIGNATURES = {
     "paraiso_hydro_version": (ctypes.c_char_p, []),
 }
 
+# the paper's linear-wave example (include/paraiso_wave.h), exported by the same library
+WAVE_SIGNATURES = {
+    "paraiso_wave_create": (_int, [ctypes.POINTER(_vp), _i64, _dbl]),
+    "paraiso_wave_destroy": (_int, [_vp]),
+    "paraiso_wave_set_state": (_int, [_vp, _vp, _vp]),
+    "paraiso_wave_get_state": (_int, [_vp, _vp, _vp]),
+    "paraiso_wave_step": (_int, [_vp, _i64, _vp]),
+    "paraiso_wave_launch_count": (_int, [_vp, _pi64]),
+}
+
 # the probe library (include/paraiso_hydro_probe.h): tests and bench.py's roofline leg only
 PROBE_PATH = os.path.join(HERE, "libparaiso_hydro_probe.so")
 PROBE_SIGNATURES = {
@@ -78,7 +88,7 @@ def load_library(path=None):
         raise ParaisoError(PARAISO_ECUDA, f"{p} not built; run `python -m paper_1204_4779_b200.build` "
                                           "(there is no CPU fallback)")
     lib = ctypes.CDLL(p)
-    for name, (res, args) in SIGNATURES.items():
+    for name, (res, args) in list(SIGNATURES.items()) + list(WAVE_SIGNATURES.items()):
         fn = getattr(lib, name)  # AttributeError if a declared symbol is not exported
         fn.restype = res
         fn.argtypes = args
@@ -292,6 +302,65 @@ class ParaisoHydro:
         return self
 
     def __exit__(self, *exc):
+        self.destroy()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+class ParaisoWave:
+    """The paper's linear-wave example (§2.3, Table 2; include/paraiso_wave.h): fp64, periodic on [0, 2 pi),
+    dx = 2 pi / n, dt = dx / c.  step(k) advances k steps on the device and returns the energy of Eq. 8 of each."""
+
+    def __init__(self, n, c=3.43):
+        self._lib = load_library()
+        self._h = _vp()
+        self.n = int(n)
+        rc = self._lib.paraiso_wave_create(ctypes.byref(self._h), self.n, float(c))
+        if rc != PARAISO_OK:
+            self._h = _vp()
+            raise ParaisoError(rc, "paraiso_wave_create failed (no CUDA device: there is no CPU fallback)" if rc == PARAISO_ECUDA
+                               else "paraiso_wave_create failed")
+        self.dx = 2.0 * np.pi / self.n
+        self.dt = self.dx / float(c)
+
+    def _check(self, rc):
+        if rc != PARAISO_OK:
+            raise ParaisoError(rc, "paraiso_wave call failed")
+
+    def set_state(self, f, g):
+        f, g = np.ascontiguousarray(f, np.float64), np.ascontiguousarray(g, np.float64)
+        if f.shape != (self.n,) or g.shape != (self.n,):
+            raise ValueError("f and g must have n elements")
+        self._check(self._lib.paraiso_wave_set_state(self._h, f.ctypes.data, g.ctypes.data))
+
+    def get_state(self):
+        f, g = np.empty(self.n), np.empty(self.n)
+        self._check(self._lib.paraiso_wave_get_state(self._h, f.ctypes.data, g.ctypes.data))
+        return f, g
+
+    def step(self, nsteps=1):
+        e = np.empty(int(nsteps))
+        self._check(self._lib.paraiso_wave_step(self._h, int(nsteps), e.ctypes.data))
+        return e
+
+    def launch_count(self):
+        k = _i64(0)
+        self._check(self._lib.paraiso_wave_launch_count(self._h, ctypes.byref(k)))
+        return k.value
+
+    def destroy(self):
+        if self._h:
+            self._lib.paraiso_wave_destroy(self._h)
+            self._h = _vp()
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
         self.destroy()
 
     def __del__(self):

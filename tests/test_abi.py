@@ -39,6 +39,22 @@ def test_library_exports_every_declared_symbol(lib):
     assert set(binding.SIGNATURES) == set(names)
 
 
+def test_library_exports_the_wave_example(lib):
+    """include/paraiso_wave.h (the paper's linear-wave example, §2.3) is exported by the same library."""
+    from paper_1204_4779_b200 import binding
+
+    text = re.sub(r"/\*.*?\*/", "", open(os.path.join(ROOT, "include", "paraiso_wave.h")).read(), flags=re.S)
+    names = sorted(set(re.findall(r"\b(paraiso_wave_[a-z_]+)\s*\(", text)))
+    assert names == sorted(binding.WAVE_SIGNATURES) and len(names) == 6
+    raw = ctypes.CDLL(binding.LIB_PATH)
+    for name in names:
+        assert hasattr(raw, name), name
+    h = ctypes.c_void_p()
+    assert lib.paraiso_wave_create(ctypes.byref(h), 2, 3.43) == binding.PARAISO_EINVAL      # n < 3
+    assert lib.paraiso_wave_create(ctypes.byref(h), 64, 0.0) == binding.PARAISO_EINVAL      # c <= 0
+    assert lib.paraiso_wave_destroy(None) == binding.PARAISO_OK
+
+
 def test_probe_library_exports_every_declared_symbol(lib):
     """include/paraiso_hydro_probe.h: the test / measurement probes live in a library of their own."""
     from paper_1204_4779_b200 import binding

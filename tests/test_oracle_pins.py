@@ -611,3 +611,52 @@ def test_p16_paper_validation_procedure_on_the_oracle(oracle_mod, problem, theta
         assert orders[-1] > 1.7 and all(b > a for a, b in zip(orders, orders[1:])), (errs, orders)
         amplitude = 1.0 if problem == "entropy" else 1.4e-5
         assert errs[-1] < 4e-3 * amplitude, errs
+
+
+# ---------------------------------------------------------------- P17: the paper's linear-wave example (§2.3)
+def _wave_ic(n, dx):
+    x = np.arange(n) * dx
+    return np.sin(x), np.cos(3 * x)  # Eq. 9-10
+
+
+@pytest.mark.parametrize("n", [8, 48, 384, 3072])
+def test_p17_wave_energy_fluctuation_is_what_the_paper_reports(oracle_mod, n):
+    """"with resolution varying from N=8 to N=3072 ... the fluctuation of discrete conserved quantity,
+    Eq. (8) was smaller than of the order of 1e-13" (c = 3.43, f = sin x, g = cos 3x, Eq. 9-10)."""
+    w = oracle_mod.Wave(n)
+    w.set_state(*_wave_ic(n, w.dx))
+    E = np.array([w.step() for _ in range(2 * n)])
+    assert (E.max() - E.min()) / E.mean() < 1e-12, (E.max() - E.min()) / E.mean()
+    # the continuum value of Eq. 5 for this initial condition: c^2/2 * pi + 1/2 * pi, approached at second order
+    exact = 0.5 * np.pi * (3.43**2 + 1.0)
+    assert abs(E[0] - exact) / exact < 40.0 / n**2 + 1e-12, (E[0], exact)
+
+
+def test_p17_wave_scheme_against_its_closed_form(oracle_mod):
+    """Eq. 6-7 with c dt = dx eliminate g:  f^{n+1}[i] + f^{n-1}[i] = f^n[i+1] + f^n[i-1]  (the exact d'Alembert update of
+    the wave equation at unit Courant number), and g^n = (f^{n+1} - f^n)/dt; first step by hand on 8 cells."""
+    n = 8
+    w = oracle_mod.Wave(n)
+    f0, g0 = _wave_ic(n, w.dx)
+    w.set_state(f0, g0)
+    hist = [f0]
+    gs = [g0]
+    for _ in range(12):
+        w.step()
+        f, g = w.get_state()
+        hist.append(f)
+        gs.append(g)
+    for k in range(1, 12):
+        lhs = hist[k + 1] + hist[k - 1]
+        rhs = np.roll(hist[k], -1) + np.roll(hist[k], 1)
+        assert np.abs(lhs - rhs).max() < 1e-13
+        assert np.abs(gs[k] - (hist[k + 1] - hist[k]) / w.dt).max() < 1e-12
+    # first step written out: f1 = f0 + dt g0; g1 = g0 + (c/dx) (f1[i-1] + f1[i+1] - 2 f1[i])   (dt c^2/dx^2 = c/dx)
+    f1 = f0 + w.dt * g0
+    g1 = g0 + (3.43 / w.dx) * (np.roll(f1, 1) + np.roll(f1, -1) - 2 * f1)
+    assert np.abs(hist[1] - f1).max() < 1e-15 and np.abs(gs[1] - g1).max() < 1e-13
+    # a constant f with g = 0 is a fixed point with zero energy; a uniform drift g = const moves f and keeps E = g^2/2 * 2 pi
+    w.set_state(np.full(n, 2.5), np.zeros(n))
+    assert w.step() == 0.0 and np.array_equal(w.get_state()[0], np.full(n, 2.5))
+    w.set_state(np.zeros(n), np.full(n, 2.0))
+    assert abs(w.step() - 0.5 * 4.0 * 2 * np.pi) < 1e-14
