@@ -92,7 +92,8 @@ int paraiso_hydro_destroy(paraiso_hydro_t *h);
  *               1 hardware reciprocal / reciprocal-square-root approximations: inside north_star's fp32 tolerances,
  *               not bit-equal, ~15 % faster (R21)
  *   "staging"   k_march only: 0 / 1 every thread loads its own cells (default) | 2 TMA bulk copies of the tile rows into a
- *               shared-memory ring (one cell per thread, n_x a multiple of 16 bytes; measured slower)
+ *               shared-memory ring (cp.async.bulk; one cell per thread, n_x a multiple of 16 bytes) | 3 the same ring
+ *               filled by one tensor-map copy per plane (cp.async.bulk.tensor); both measured, DESIGN.md §7
  *   "integrator" 0 the paper's two-stage midpoint rule, Eq. 24-27 (default) | 1 Heun / Shu-Osher SSP-RK2, the
  *               "2-stage TVD Runge-Kutta" north_star names as the fallback (R20): same kernels and traffic
  *   "state_kind" 0 set_state / get_state exchange conserved variables U = (rho, m_a, E) (default) |

@@ -23,6 +23,10 @@
 // outside [0, n) holds the state of a mapped cell (wrap or clamp); threads whose own cells lie outside the grid
 // compute but never store.  T = f32x2 needs an even n_x (the launcher falls back to T = float otherwise).
 #pragma once
+#include <cuda.h>  // CUtensorMap (the descriptor of the tensor-map TMA staging, TMA = 2)
+
+#include <cstring>
+
 #include "hydro_kernels_basic.cuh"
 
 // blocks per SM the register cap of __launch_bounds__ is set for: fp32 one cell per thread (two 256-thread blocks,
@@ -95,7 +99,8 @@ __device__ __forceinline__ int bad_lanes(const Prim<T, D>& V, T E) {
   return lane_count(m_or(m_or(m_not(gt(V.rho, zero)), m_not(gt(V.p, zero))), m_not(le(rabs(E), T(S(3.0e38))))));
 }
 
-template <class T, int D, int NWX, int TY, bool TMA = false, int RPT = 1>
+// TMA: 0 none | 1 bulk row copies (cp.async.bulk, SASS UBLKCP) | 2 one tensor-map copy per plane (cp.async.bulk.tensor, UTMALDG)
+template <class T, int D, int NWX, int TY, int TMA = 0, int RPT = 1>
 struct MarchShape {
   using S = scalar_t<T>;
   static constexpr int W = LaneTraits<T>::W;
@@ -220,10 +225,24 @@ __device__ __forceinline__ void tma_row(void* dst, const void* src, int bytes, u
 
 __device__ __forceinline__ void block_barrier() { asm volatile("bar.sync 0;" ::: "memory"); }
 
-template <class T, int D, int RS, int STAGE, int NWX, int TY, int MINB, bool TMA, int RPT>
+// global -> shared, one box of a tensor map (cp.async.bulk.tensor: SASS UTMALDG); rank 3 (x, y, f) or 4 (x, y, z, f)
+__device__ __forceinline__ void tma_box3(void* dst, const CUtensorMap* tm, int c0, int c1, int c2, unsigned long long* bar) {
+  asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(
+                   smem_addr(dst)),
+               "l"(reinterpret_cast<unsigned long long>(tm)), "r"(c0), "r"(c1), "r"(c2), "r"(smem_addr(bar))
+               : "memory");
+}
+__device__ __forceinline__ void tma_box4(void* dst, const CUtensorMap* tm, int c0, int c1, int c2, int c3, unsigned long long* bar) {
+  asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];" ::"r"(
+                   smem_addr(dst)),
+               "l"(reinterpret_cast<unsigned long long>(tm)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_addr(bar))
+               : "memory");
+}
+
+template <class T, int D, int RS, int STAGE, int NWX, int TY, int MINB, int TMA, int RPT>
 __global__ void __launch_bounds__(MarchShape<T, D, NWX, TY, TMA, RPT>::NT, MINB)
     k_march(const scalar_t<T>* __restrict__ Uin, const scalar_t<T>* Ubase, scalar_t<T>* Uout, Geom<scalar_t<T>> g,
-            Scalars* sc, int depth) {
+            Scalars* sc, int depth, const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUtensorMap tm_base) {
   using Sh = MarchShape<T, D, NWX, TY, TMA, RPT>;
   using S = scalar_t<T>;
   using P = Prim<T, D>;
@@ -248,7 +267,8 @@ __global__ void __launch_bounds__(MarchShape<T, D, NWX, TY, TMA, RPT>::NT, MINB)
   auto grid_row = [&](int gj) { return (D == 3) ? march_src(gj, ny, bnd) * nx : 0; };
 
   // TMA staging needs whole, 16-byte aligned rows: tiles that end inside the grid (the launcher checks n_x % 4)
-  const bool use_tma = TMA && (x0 + TXC <= nx);
+  // (TMA = 2: a box does not wrap, so the tile's rows must lie inside the grid as well)
+  const bool use_tma = TMA && (x0 + TXC <= nx) && (TMA == 1 || D == 2 || y0 + TYC <= ny);
 
   S s_max = S(0);
   int bad = 0;
@@ -561,12 +581,23 @@ __global__ void __launch_bounds__(MarchShape<T, D, NWX, TY, TMA, RPT>::NT, MINB)
       job_off[j] = job < NJOB ? f * Ni + grid_row(y0 + r) + x0 : -1;
     }
     auto tma_plane = [&](const S* A, int m, S* dst_slot, unsigned long long* bar) {
-      const int pl = plane_of(m);
-      if (lane == 0) mbar_expect_tx(bar, NJOB * ROW_BYTES);
-      __syncwarp();
+      if constexpr (TMA == 2) {  // one instruction per plane: the box (TXC, rows, 1 plane, NF fields) of the tensor map
+        if (lane == 0) {
+          mbar_expect_tx(bar, NJOB * ROW_BYTES);
+          const CUtensorMap* tm = (A == Uin) ? &tm_in : &tm_base;
+          const int pm = map_index(m, nM, bnd);
+          if constexpr (D == 3) tma_box4(dst_slot, tm, x0, y0, pm, 0, bar);
+          else tma_box3(dst_slot, tm, x0, pm, 0, bar);
+        }
+        __syncwarp();
+      } else {
+        const int pl = plane_of(m);
+        if (lane == 0) mbar_expect_tx(bar, NJOB * ROW_BYTES);
+        __syncwarp();
 #pragma unroll
-      for (int j = 0; j < JPL; ++j)
-        if (job_off[j] >= 0) tma_row(dst_slot + (size_t)(lane + 32 * j) * TXC, A + (job_off[j] + pl), ROW_BYTES, bar);
+        for (int j = 0; j < JPL; ++j)
+          if (job_off[j] >= 0) tma_row(dst_slot + (size_t)(lane + 32 * j) * TXC, A + (job_off[j] + pl), ROW_BYTES, bar);
+      }
     };
     if (TMA && use_tma) {
       if (lane == 0) {
@@ -648,7 +679,42 @@ __global__ void __launch_bounds__(MarchShape<T, D, NWX, TY, TMA, RPT>::NT, MINB)
 }
 
 // ------------------------------------------------------------------------------------------------
-template <class T, int D, int RS, int STAGE, int NWX, int TY, int MINB, bool TMA = false, int RPT = 1>
+// The tensor map of one state buffer: rank D + 1 (x, y[, z], field), box = (TXC, tile rows[, 1 plane], all fields).
+template <class S, int D>
+static bool make_state_tensor_map(CUtensorMap* tm, const S* U, const Geom<S>& g, int txc, int rows) {
+  typedef CUresult (*Encode)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                             const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                             CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  static Encode encode = nullptr;
+  if (!encode) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess || !p)
+      return false;
+    encode = (Encode)p;
+  }
+  constexpr int R = D + 1;
+  cuuint64_t dims[4], strides[3];
+  cuuint32_t box[4], estr[4] = {1, 1, 1, 1};
+  const cuuint64_t w = sizeof(S);
+  dims[0] = g.n[0];
+  box[0] = txc;
+  if (D == 3) {
+    dims[1] = g.n[1], dims[2] = g.n[2], dims[3] = D + 2;
+    strides[0] = g.n[0] * w, strides[1] = (cuuint64_t)g.n[0] * g.n[1] * w, strides[2] = (cuuint64_t)g.N * w;
+    box[1] = rows, box[2] = 1, box[3] = D + 2;
+  } else {
+    dims[1] = g.n[1], dims[2] = D + 2;
+    strides[0] = g.n[0] * w, strides[1] = (cuuint64_t)g.N * w;
+    box[1] = 1, box[2] = D + 2;
+  }
+  return encode(tm, sizeof(S) == 4 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64, R, (void*)U, dims,
+                strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+template <class T, int D, int RS, int STAGE, int NWX, int TY, int MINB, int TMA = 0, int RPT = 1>
 static bool launch_march_shape(const scalar_t<T>* Uin, const scalar_t<T>* Ubase, scalar_t<T>* Uout,
                                const Geom<scalar_t<T>>& g, Scalars* sc, cudaStream_t stream, int depth) {
   using Sh = MarchShape<T, D, NWX, TY, TMA, RPT>;
@@ -674,7 +740,16 @@ static bool launch_march_shape(const scalar_t<T>* Uin, const scalar_t<T>* Ubase,
     grid.z = 1;
     if (grid.y > 65535u) return false;
   }
-  kern<<<grid, block, sizeof(typename Sh::Smem), stream>>>(Uin, Ubase, Uout, g, sc, depth);
+  CUtensorMap tm_in, tm_base;
+  if constexpr (TMA == 2) {
+    if (!make_state_tensor_map<scalar_t<T>, D>(&tm_in, Uin, g, Sh::TXC, Sh::XROWS) ||
+        !make_state_tensor_map<scalar_t<T>, D>(&tm_base, Ubase, g, Sh::TXC, Sh::XROWS))
+      return false;
+  } else {
+    memset(&tm_in, 0, sizeof tm_in);
+    memset(&tm_base, 0, sizeof tm_base);
+  }
+  kern<<<grid, block, sizeof(typename Sh::Smem), stream>>>(Uin, Ubase, Uout, g, sc, depth, tm_in, tm_base);
   return true;
 }
 
@@ -694,7 +769,8 @@ inline int march_default_depth(long long tiles_in_plane, int nM) {
 //   arith: 1 = fp32 with the hardware reciprocal / reciprocal square root approximations (f32fast: inside north_star's
 //          tolerances, not bit-equal to the oracle; default shapes only), 0 = IEEE-exact (default)
 //   staging: 0 / 1 = every thread loads its own cells (LDG), 2 = TMA bulk copies of the tile rows into a shared-memory
-//            ring (one cell per thread, n_x a multiple of 16 bytes, default tile shapes only)
+//            ring (one cell per thread, n_x a multiple of 16 bytes, default tile shapes only), 3 = the same ring filled by
+//            ONE tensor-map copy per plane (cp.async.bulk.tensor: SASS UTMALDG)
 template <class Real, int D, int RS, int STAGE>
 bool launch_march_stage(const Real* Uin, const Real* Ubase, Real* Uout, const Geom<Real>& g, Scalars* sc,
                         cudaStream_t stream, const int* block, int tile_depth, int pack, int staging, int arith) {
@@ -707,6 +783,7 @@ bool launch_march_stage(const Real* Uin, const Real* Ubase, Real* Uout, const Ge
     if (pack == 2 && !packed) return false;
     const int w = packed ? 2 : 1;
     const bool tma = staging == 2 && !packed && g.n[0] % (16 / (int)sizeof(Real)) == 0;
+    const bool tma_map = staging == 3 && !packed && g.n[0] % (16 / (int)sizeof(Real)) == 0;  // tensor-map TMA
     if constexpr (D == 2) {
       int nwx = block[0] > 0 ? block[0] : 4;
       const long long tiles = (g.n[0] + nwx * 32 * w - 1) / (nwx * 32 * w);
@@ -719,7 +796,8 @@ bool launch_march_stage(const Real* Uin, const Real* Ubase, Real* Uout, const Ge
   }
       if constexpr (can_pack)
         if (arith == 1 && nwx == 4) return launch_march_shape<f32fast, D, RS, STAGE, 4, 1, minb>(Uin, Ubase, Uout, g, sc, stream, depth);
-      if (tma && nwx == 4) return launch_march_shape<Real, D, RS, STAGE, 4, 1, minb, true>(Uin, Ubase, Uout, g, sc, stream, depth);
+      if (tma && nwx == 4) return launch_march_shape<Real, D, RS, STAGE, 4, 1, minb, 1>(Uin, Ubase, Uout, g, sc, stream, depth);
+      if (tma_map && nwx == 4) return launch_march_shape<Real, D, RS, STAGE, 4, 1, minb, 2>(Uin, Ubase, Uout, g, sc, stream, depth);
       PH_SHAPE(2) PH_SHAPE(3) PH_SHAPE(4) PH_SHAPE(7) PH_SHAPE(8)
 #undef PH_SHAPE
       return false;
@@ -735,9 +813,10 @@ bool launch_march_stage(const Real* Uin, const Real* Ubase, Real* Uout, const Ge
   }
       if constexpr (can_pack)
         if (arith == 1 && ty == 7) return launch_march_shape<f32fast, D, RS, STAGE, 1, 7, minb>(Uin, Ubase, Uout, g, sc, stream, depth);
-      if (tma && ty == 7) return launch_march_shape<Real, D, RS, STAGE, 1, 7, minb, true>(Uin, Ubase, Uout, g, sc, stream, depth);
+      if (tma && ty == 7) return launch_march_shape<Real, D, RS, STAGE, 1, 7, minb, 1>(Uin, Ubase, Uout, g, sc, stream, depth);
+      if (tma_map && ty == 7) return launch_march_shape<Real, D, RS, STAGE, 1, 7, minb, 2>(Uin, Ubase, Uout, g, sc, stream, depth);
       if (block[2] == 2 && ty == 7 && !packed)  // two rows per thread: a 32 x 14 tile, one 256-thread block per SM
-        return launch_march_shape<Real, D, RS, STAGE, 1, 7, PH_RPT2_MINB, false, 2>(Uin, Ubase, Uout, g, sc, stream, depth);
+        return launch_march_shape<Real, D, RS, STAGE, 1, 7, PH_RPT2_MINB, 0, 2>(Uin, Ubase, Uout, g, sc, stream, depth);
       PH_SHAPE(4) PH_SHAPE(7) PH_SHAPE(8) PH_SHAPE(15)
 #undef PH_SHAPE
       return false;

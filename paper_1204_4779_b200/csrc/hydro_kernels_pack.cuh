@@ -264,21 +264,30 @@ __global__ void __launch_bounds__(PackShape<T, D, NWX, TY, NH>::NT, MINB)
           for (int f = 0; f < NF; ++f) sts(&sm.Fy[f][row + 1][c0], Fy[f]);
         }
       }
+      // own-cell base state of Eq. 23 and the x flux of the left neighbour lane: both this thread's / warp's own data,
+      // fetched before the barrier so that only the other warps' results are waited for after it
+      cp_async_wait_all();
+      T ub[NF];
+      S nbx[NF];
+#pragma unroll
+      for (int f = 0; f < NF; ++f) {
+        ub[f] = lds<T>(&sm.Ub[f][row][c0]);
+        nbx[f] = shfl_up(lane_last(Fx[f]));
+      }
       block_barrier();
 
       // ------------------------------------------------------------ phase C: Eq. 23, axes in the order x, y, z
       T lowx[NF];
 #pragma unroll
       for (int f = 0; f < NF; ++f) {
-        S nb = shfl_up(lane_last(Fx[f]));
+        S nb = nbx[f];
         if (lane == 0) nb = sm.Fx[f][row][wx];
         lowx[f] = xshift_left(Fx[f], nb);
       }
-      cp_async_wait_all();
       if (active) {
         T u[NF];  // own-cell base state of Eq. 23 (copied in phase A; U_base is overwritten in place only below)
 #pragma unroll
-        for (int f = 0; f < NF; ++f) u[f] = rfma(lam0, lowx[f] - Fx[f], lds<T>(&sm.Ub[f][row][c0]));
+        for (int f = 0; f < NF; ++f) u[f] = rfma(lam0, lowx[f] - Fx[f], ub[f]);
         if constexpr (D == 3) {
 #pragma unroll
           for (int f = 0; f < NF; ++f) u[f] = rfma(lam1, lds<T>(&sm.Fy[f][row][c0]) - Fy[f], u[f]);
@@ -458,7 +467,8 @@ __global__ void __launch_bounds__(PackShape<T, D, NWX, TY, NH>::NT, MINB)
 // ------------------------------------------------------------------------------------------------
 // Planes marched per block when the caller gives none.  A block pays a prologue of about two planes' work, and the
 // grid runs in waves of `capacity` blocks: the depth (8 .. 128) is the one that wastes least of both, i.e. maximises
-// (blocks / (waves * capacity)) * depth / (depth + 2); ties go to the deeper march.
+// (blocks / (waves * capacity)) * depth / (depth + 2) * waves / (waves + 0.1); the last factor is the measured
+// preference for a few waves over exactly one (the tuner tables of configs 2 and 3); ties go to the deeper march.
 inline int pack_default_depth(long long tiles_in_plane, int nM, int capacity) {
   int best = 8;
   double best_eff = -1.0;
@@ -466,7 +476,7 @@ inline int pack_default_depth(long long tiles_in_plane, int nM, int capacity) {
     const int depth = (nM + zb - 1) / zb;
     const long long blocks = tiles_in_plane * ((nM + depth - 1) / depth);
     const long long waves = (blocks + capacity - 1) / capacity;
-    const double eff = double(blocks) / double(waves * capacity) * depth / (depth + 2.0);
+    const double eff = double(blocks) / double(waves * capacity) * depth / (depth + 2.0) * double(waves) / (double(waves) + 0.1);
     if (eff > best_eff * 1.0001) {
       best_eff = eff;
       best = depth;

@@ -83,7 +83,7 @@ struct paraiso_hydro {
   int block[3] = {0, 0, 0};
   int tile_depth = 0, cells_per_thread = 0, use_graph = 1;
   int arith = 0;       // k_march fp32: 0 IEEE-exact division / square root, 1 hardware approximations (f32fast)
-  int staging = 0;     // k_march: 0 / 1 own-cell LDG, 2 TMA bulk copies into a shared-memory ring
+  int staging = 0;     // k_march: 0 / 1 own-cell LDG, 2 TMA bulk row copies into a shared-memory ring, 3 one tensor-map copy per plane
   int integrator = 0;  // 0 midpoint (paper) | 1 Heun
   int limiter = 0;     // 0 MINBEE (Eq. 21) | 1 none (first order) | 2 monotonized central (R22): k_pack, k_delayed
   int state_kind = 0;  // 0: set_state / get_state exchange conserved variables, 1: primitive variables
@@ -527,7 +527,7 @@ static bool find_option(paraiso_hydro* h, const char* key, OptionRef* ref) {
                       {"state_kind", {&h->state_kind, 0, 1}},
                       {"integrator", {&h->integrator, 0, 1}},
                       {"limiter", {&h->limiter, 0, 2}},
-                      {"staging", {&h->staging, 0, 2}},
+                      {"staging", {&h->staging, 0, 3}},
                       {"arith", {&h->arith, 0, 1}},
                       {"kernel_used", {&h->kernel_used, 0, 0}}};  // read-only: KERNEL_* of the last stage launch
   for (const Opt& o : opts)

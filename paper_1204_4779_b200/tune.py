@@ -42,6 +42,7 @@ def candidates(dims, dtype_is_f32):
             for ty in (7, 8):
                 out.append((f"march packed f32x2 ty={ty}", "march", {"block_y": ty, "cells_per_thread": 2}))
         out.append(("march ty=7 TMA staging", "march", {"block_y": 7, "staging": 2}))
+        out.append(("march ty=7 tensor-map TMA staging", "march", {"block_y": 7, "staging": 3}))
         out.append(("march ty=7 two rows per thread", "march", {"block_y": 7, "block_z": 2}))
         if dtype_is_f32:
             out.append(("march ty=7 arith=1 (not bit-equal)", "march", {"block_y": 7, "arith": 1}))
@@ -53,6 +54,7 @@ def candidates(dims, dtype_is_f32):
         if dtype_is_f32:
             out.append(("march packed f32x2 warps=4", "march", {"block_x": 4, "cells_per_thread": 2}))
         out.append(("march warps=4 TMA staging", "march", {"block_x": 4, "staging": 2}))
+        out.append(("march warps=4 tensor-map TMA staging", "march", {"block_x": 4, "staging": 3}))
         if dtype_is_f32:
             out.append(("march warps=4 arith=1 (not bit-equal)", "march", {"block_x": 4, "arith": 1}))
     return out

@@ -436,9 +436,9 @@ def test_march_tma_staging_matches_oracle(gpu, oracle_mod, dims, shape, boundary
     for dtype in (np.float32, np.float64):
         w = inputs.random_smooth(shape, dtype, seed=41 + dims, boundary=boundary)
         ref, rdt = oracle_steps(oracle_mod, w, 3)
-        for depth in (0, 5):
-            got, gdt = gpu_steps(gpu, w, 3, "march", staging=2, tile_depth=depth)
-            assert np.array_equal(got, ref), (shape, dtype, depth, field_errors(got, ref))
+        for depth, staging in ((0, 2), (5, 2), (0, 3), (5, 3)):  # 2: bulk row copies, 3: one tensor-map copy per plane
+            got, gdt = gpu_steps(gpu, w, 3, "march", staging=staging, tile_depth=depth)
+            assert np.array_equal(got, ref), (shape, dtype, depth, staging, field_errors(got, ref))
             assert all(abs(a - b) <= TOL[np.dtype(dtype)][2] * b for a, b in zip(gdt, rdt))
 
 
