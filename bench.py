@@ -480,6 +480,10 @@ def main():
         # this device: the model DESIGN.md §8 reads the ncu captures with
         mhz = (clocks or {}).get("sm_mhz") or 1965.0
         line["roofline"]["issue_cost_cycles"] = {k: round(binding.probe_issue_cost(k, mhz)[0], 3) for k in binding.ISSUE_KINDS}
+        # the issue rate the default stage kernel's instruction mix reaches with NO dependencies (4 warps per scheduler):
+        # the ceiling its ncu-measured issue rate (profiles/r2_ncu_summary.txt: 0.51-0.53) is to be read against
+        line["roofline"]["mix_ceiling_ipc"] = {"k_pack_mix_packed": round(binding.probe_mix_ceiling(0, mhz), 3),
+                                               "same_work_scalar_ffma": round(binding.probe_mix_ceiling(1, mhz), 3)}
     if rank == 0 and not args.no_sweep:
         line["all_configs"] = sweep(binding, torch, args, peak, peak_src)
     if rank == 0 and not args.no_cpu:

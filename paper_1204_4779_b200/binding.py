@@ -65,6 +65,7 @@ PROBE_SIGNATURES = {
     "paraiso_probe_arith": (_int, [_int, _i64, _vp, _vp, _vp, _vp]),
     "paraiso_probe_issue_cost": (_int, [_int, _dbl, _pdbl, _pdbl]),
     "paraiso_probe_peak": (_int, [_int, _pdbl]),
+    "paraiso_probe_mix_ceiling": (_int, [_int, _dbl, _pdbl]),
 }
 
 _LIB = None
@@ -149,6 +150,16 @@ def probe_peak(kind):
     rc = load_probe().paraiso_probe_peak(PEAK_KINDS[kind] if isinstance(kind, str) else int(kind), ctypes.byref(v))
     if rc:
         raise ParaisoError(rc, "probe_peak failed")
+    return v.value
+
+
+def probe_mix_ceiling(mix, sm_clock_mhz):
+    """paraiso_probe_mix_ceiling: warp instructions per cycle per scheduler of the stage kernel's instruction mix without
+    dependencies (mix 0: packed, as k_pack; 1: scalar FFMA)."""
+    v = _dbl(0)
+    rc = load_probe().paraiso_probe_mix_ceiling(int(mix), float(sm_clock_mhz), ctypes.byref(v))
+    if rc != 0:
+        raise ParaisoError(rc, "probe_mix_ceiling failed")
     return v.value
 
 

@@ -24,6 +24,10 @@
 #ifndef PH_PACK64_MINB2
 #define PH_PACK64_MINB2 4
 #endif
+// fp32, 2-D rows: likewise
+#ifndef PH_PACK32_MINB2
+#define PH_PACK32_MINB2 2
+#endif
 
 namespace ph {
 
@@ -561,7 +565,7 @@ bool launch_pack_stage(const Real* Uin, const Real* Ubase, Real* Uout, const Geo
         if (halo_warp) nwx = 4;
       }
       const int depth = tile_depth;  // 0: launch_pack_bnd picks it from the kernel's occupancy
-      constexpr int MB = F32 ? 2 : PH_PACK64_MINB2;
+      constexpr int MB = F32 ? PH_PACK32_MINB2 : PH_PACK64_MINB2;
       if (!halo_warp) {
         if constexpr (F32)
           if (nwx == 1) return launch_pack_shape<T, D, RS, STAGE, 1, 1, MB, 0>(Uin, Ubase, Uout, g, sc, stream, depth);

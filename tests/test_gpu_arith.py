@@ -79,3 +79,16 @@ def test_measured_peak_lane_rates():
     assert 0.5 * nominal <= pk["ffma"] <= 1.05 * nominal
     assert 0.7 * nominal <= pk["ffma2"] <= 1.05 * nominal
     assert 0.25 * nominal <= pk["dfma"] <= 0.55 * nominal
+
+
+def test_mix_ceiling_probe():
+    """paraiso_probe_mix_ceiling: the stage kernel's instruction mix without dependencies issues well below one
+    instruction per cycle on four warps per scheduler (the packed FMA and the ALU instructions each hold their pipe for
+    two cycles): the ceiling DESIGN.md §8 reads the kernel's 0.51-0.53 against."""
+    from paper_1204_4779_b200 import binding
+
+    packed = binding.probe_mix_ceiling(0, 1965.0)
+    scalar = binding.probe_mix_ceiling(1, 1965.0)
+    print(f"mix ceiling: packed {packed:.3f} IPC (76 instructions), scalar {scalar:.3f} IPC (108 instructions)")
+    assert 0.55 < packed < 0.9 and 0.7 < scalar < 1.01
+    assert 76.0 / packed < 108.0 / scalar  # the packed mix still finishes the same work sooner
