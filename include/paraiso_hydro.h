@@ -67,7 +67,8 @@ int paraiso_hydro_destroy(paraiso_hydro_t *h);
  *   "variant"   kernel arrangement on the paper's Manifest <-> Delayed axis (Table 5):
  *               0 fused       one kernel per RK stage, intermediates on chip (default): k_pack on 2-D and 3-D grids
  *                             (fp32: packed pairs of cells, needs an even n_x, else k_march; fp64: one cell per
- *                             thread), k_delayed in 1-D
+ *                             thread); in 1-D k_small1d up to 1024 cells (any number of steps in ONE launch, the
+ *                             state in registers), k_delayed beyond
  *               6 pack        force k_pack (marching window in shared memory; the fastest on-chip kernel)
  *               4 march       force k_march (marching window in registers; "cells_per_thread" 2 = packed f32x2)
  *               5 fused1      force k_fused (the first on-chip design)

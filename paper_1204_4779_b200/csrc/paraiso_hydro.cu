@@ -13,6 +13,7 @@
 #include "hydro_kernels_fused.cuh"
 #include "hydro_kernels_march.cuh"
 #include "hydro_kernels_pack.cuh"
+#include "hydro_kernels_small.cuh"
 
 using namespace ph;
 
@@ -69,7 +70,7 @@ PH_EXTERN_LIM(double, 3)
 enum { VARIANT_FUSED = 0, VARIANT_MANIFEST_FLUX = 1, VARIANT_MANIFEST_ALL = 2, VARIANT_DELAYED = 3, VARIANT_MARCH = 4,
        VARIANT_FUSED1 = 5, VARIANT_PACK = 6 };
 enum { KERNEL_NONE = 0, KERNEL_MANIFEST_FLUX = 1, KERNEL_MANIFEST_ALL = 2, KERNEL_DELAYED = 3, KERNEL_MARCH = 4,
-       KERNEL_FUSED1 = 5, KERNEL_PACK = 6 };
+       KERNEL_FUSED1 = 5, KERNEL_PACK = 6, KERNEL_SMALL1D = 7 };
 
 struct paraiso_hydro {
   int dims = 0, dtype = 0, nf = 0;
@@ -380,6 +381,27 @@ struct Launch {
     stage<2>(h);
   }
 
+  // 1-D grids of at most 1024 cells, default variant: `nsteps` whole steps in ONE launch (hydro_kernels_small.cuh)
+  static bool small_run_covers(const paraiso_hydro* h) {
+    return D == 1 && h->variant == VARIANT_FUSED && h->N <= SMALL1D_MAX && !h->timing && !h->block[0] && !h->block[1] &&
+           !h->block[2] && !h->tile_depth && !h->cells_per_thread && !h->staging && !h->arith;
+  }
+  static void small_run(paraiso_hydro* h, int64_t nsteps) {
+    if constexpr (D == 1) {
+      const Geom<Real> g = make_geom<Real>(h);
+      const int bs = int((h->N + 31) / 32 * 32);
+      Real* U = (Real*)h->U[0];
+      if (h->limiter == LIMITER_NONE)
+        k_small1d<Real, RS, LIMITER_NONE><<<1, bs, 0, h->stream>>>(U, g, h->sc, (long long)nsteps);
+      else if (h->limiter == LIMITER_MC)
+        k_small1d<Real, RS, LIMITER_MC><<<1, bs, 0, h->stream>>>(U, g, h->sc, (long long)nsteps);
+      else
+        k_small1d<Real, RS, LIMITER_MINBEE><<<1, bs, 0, h->stream>>>(U, g, h->sc, (long long)nsteps);
+      h->launches += 1;
+      h->kernel_used = KERNEL_SMALL1D;
+    }
+  }
+
   static void cfl(paraiso_hydro* h) {
     const Geom<Real> g = make_geom<Real>(h);
     const int bs = 256;
@@ -616,7 +638,10 @@ int paraiso_hydro_step(paraiso_hydro_t* h, double dt) {
   if (rc) return rc;
   dispatch(h, [&](auto L) {
     L.control(h, CTRL_MANUAL_DT, dt, 0);
-    L.step(h);
+    if (L.small_run_covers(h))
+      L.small_run(h, 1);
+    else
+      L.step(h);
   });
   return check_launch(h);
 }
@@ -699,6 +724,12 @@ static int64_t launches_per_step(const paraiso_hydro* h) {
 }
 
 static int enqueue_steps(paraiso_hydro* h, int64_t nsteps) {
+  bool small = false;
+  dispatch(h, [&](auto L) { small = L.small_run_covers(h); });
+  if (small) {  // the whole chunk of steps in one launch
+    if (nsteps > 0) dispatch(h, [&](auto L) { L.small_run(h, nsteps); });
+    return check_launch(h);
+  }
   const int chunk = 8;  // steps per graph
   int64_t left = nsteps;
   if (h->use_graph && !h->timing && nsteps >= chunk) {

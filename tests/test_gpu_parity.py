@@ -293,7 +293,7 @@ def test_pack_launch_shapes_match_oracle(gpu, oracle_mod, dims, opts, boundary):
             assert np.array_equal(got, ref), "the packed kernel states the same arithmetic as the oracle: bit-equal"
 
 
-KERNEL_ID = {"manifest_flux": 1, "manifest_all": 2, "delayed": 3, "march": 4, "fused1": 5, "pack": 6}
+KERNEL_ID = {"manifest_flux": 1, "manifest_all": 2, "delayed": 3, "march": 4, "fused1": 5, "pack": 6, "small1d": 7}
 
 
 def test_uncovered_shapes_are_errors(gpu, oracle_mod):
@@ -523,7 +523,8 @@ def test_limiter_option_matches_oracle(gpu, oracle_mod, dims, dtype, limiter):
                 got = h.get_state()
                 tg, kg = h.time()
                 assert h.stats() == 0 and kg == 11
-                assert h.get_option("kernel_used") == KERNEL_ID["delayed" if (variant == "delayed" or dims == 1) else "pack"]
+                want = "delayed" if variant == "delayed" else ("small1d" if dims == 1 else "pack")  # 1-D, <= 1024 cells: one launch
+                assert h.get_option("kernel_used") == KERNEL_ID[want]
             assert abs(tg - t) <= 20 * TOL[np.dtype(dtype)][2] * t
             assert np.array_equal(got, ref), (variant, boundary, field_errors(got, ref))
     # the slopes really are off / different: the three variants give three different states
@@ -571,3 +572,41 @@ def test_prescribed_ghost_cells_match_oracle(gpu, oracle_mod, dims, dtype, varia
         assert h.time()[1] == 3
     assert np.array_equal(got, o.get_state()), field_errors(got, o.get_state())
     o.close()
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("n", [4, 5, 31, 256, 1000, 1024])
+def test_small_1d_grids_run_in_one_launch(gpu, oracle_mod, n, dtype):
+    """1-D grids of at most 1024 cells (BASELINE config 0), default variant: k_small1d advances any number of steps in
+    ONE kernel launch (state in registers, time-step control on the device).  Bit-equal to the oracle for both Riemann
+    solvers, both boundaries and integrators, stepped by hand, device-paced, and to a t_end; 1025 cells take k_delayed."""
+    for boundary, riemann, integ in (("outflow", "hllc", 0), ("periodic", "hll", 0), ("periodic", "hllc", 1)):
+        w = inputs.random_smooth((n,), dtype, seed=90 + n, boundary=boundary)
+        o = oracle_mod.Oracle(w.n, w.extent, w.gamma, w.dtype, boundary, riemann, "serial", "heun" if integ else "midpoint")
+        o.set_state(w.U)
+        for _ in range(2):
+            o.step(o.cfl_dt(w.cfl))
+        k, t = o.run(w.cfl, 37)
+        k2, t2 = o.run(w.cfl, 10**6, t + 0.01)
+        ref = o.get_state()
+        o.close()
+        with gpu.ParaisoHydro(w.n, w.extent, w.gamma, w.dtype, boundary, riemann, integrator=integ) as h:
+            h.set_state(w.U)
+            for _ in range(2):
+                h.step(h.cfl_dt(w.cfl))
+            l0 = h.launch_count()
+            h.run(w.cfl, 37)
+            assert h.launch_count() - l0 == 2  # the control kernel + ONE stage kernel for 37 steps
+            assert h.get_option("kernel_used") == KERNEL_ID["small1d"]
+            tg, kg = h.time()
+            assert kg == 39 and abs(tg - t) <= 50 * TOL[np.dtype(dtype)][2] * t
+            kk, tt = h.run(w.cfl, 10**6, t + 0.01)
+            assert kk == k2 and tt == t + 0.01
+            got = h.get_state()
+            assert h.stats() == 0
+        assert np.array_equal(got, ref), (n, boundary, riemann, integ, field_errors(got, ref))
+    w = inputs.random_smooth((1025,), dtype, seed=3)
+    with gpu.ParaisoHydro(w.n, w.extent, w.gamma, w.dtype) as h:
+        h.set_state(w.U)
+        h.run(w.cfl, 3)
+        assert h.get_option("kernel_used") == KERNEL_ID["delayed"]
