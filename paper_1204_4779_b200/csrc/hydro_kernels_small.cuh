@@ -15,9 +15,14 @@ template <class Real, int RS, int LIM>
 __global__ void __launch_bounds__(SMALL1D_MAX) k_small1d(Real* U, Geom<Real> g, Scalars* sc, long long nsteps) {
   constexpr int D = 1, NF = 3;
   __shared__ Real Vs[NF][SMALL1D_MAX];
+  __shared__ Scalars lsc;  // the handle's scalar block, kept on chip for the whole run and written back at the end
+  __shared__ Real s_warp[32];
+  __shared__ int s_bad[32];
   const int n = g.n[0], i = threadIdx.x, bnd = g.boundary;
   const bool cell = i < n;
-  volatile Scalars* vsc = sc;
+  if (i == 0) lsc = *sc;
+  __syncthreads();
+  volatile Scalars* vsc = &lsc;
   Real u0[NF] = {Real(1), Real(0), Real(1)};
   if (cell) load_fields_rw<Real, NF>(U, g.N, i, u0);
 
@@ -74,11 +79,35 @@ __global__ void __launch_bounds__(SMALL1D_MAX) k_small1d(Real* U, Geom<Real> g, 
       smax = cfl_speed<Real, D>(V, ir, g.gamma, g.idr);
       bad = bad_state<Real, D>(V, u0[NF - 1]);
     }
-    block_reduce_and_finalize<Real>(smax, bad, sc, g, 1, 1);  // S, t, the step counter and the next dt on the device
-    __threadfence();
+    // a0 and the time-step control of hydro_control.cuh for ONE block: lanes by butterfly, warps through shared memory,
+    // thread 0 finishes the step (S, t, the step counter) and plans the next dt, all in the on-chip copy
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      smax = rmax(smax, __shfl_xor_sync(0xffffffffu, smax, o));
+      bad += __shfl_xor_sync(0xffffffffu, bad, o);
+    }
+    if ((i & 31) == 0) {
+      s_warp[i >> 5] = smax;
+      s_bad[i >> 5] = bad;
+    }
+    __syncthreads();
+    if (i == 0) {
+      Real S = Real(0);
+      int nb = 0;
+      for (int w = 0; w < (int)(blockDim.x >> 5); ++w) {
+        S = rmax(S, s_warp[w]);
+        nb += s_bad[w];
+      }
+      lsc.S_last = double(S);
+      lsc.nonfinite += nb;
+      lsc.t = lsc.last ? lsc.t_end : lsc.t + lsc.dt;
+      lsc.steps += 1;
+      if (lsc.auto_dt) plan_next_step(&lsc, g);
+    }
     __syncthreads();
   }
   if (cell) store_fields<Real, NF>(U, g.N, i, u0);
+  if (i == 0) *sc = lsc;
 }
 
 }  // namespace ph
