@@ -474,11 +474,16 @@ __global__ void __launch_bounds__(PackShape<T, D, NWX, TY, NH>::NT, MINB)
 // (blocks / (waves * capacity)) * depth / (depth + 2) * waves / (waves + 0.1); the last factor is the measured
 // preference for a few waves over exactly one (the tuner tables of configs 2 and 3); ties go to the deeper march.
 inline int pack_default_depth(long long tiles_in_plane, int nM, int capacity) {
-  int best = 8;
+  int best = nM < 8 ? nM : 8;
   double best_eff = -1.0;
-  for (int zb = (nM + 127) / 128; zb <= (nM + 7) / 8; ++zb) {
-    const int depth = (nM + zb - 1) / zb;
-    const long long blocks = tiles_in_plane * ((nM + depth - 1) / depth);
+  int last = 0;
+  for (int d = nM < 128 ? nM : 128; d >= 8; --d) {  // deepest first: ties go to the deeper march
+    const long long zb = (nM + d - 1) / d;  // marching blocks, then the depth that divides the axis evenly among them
+    if (zb > 65535) break;                  // the grid dimension that counts them
+    const int depth = int((nM + zb - 1) / zb);
+    if (depth == last) continue;
+    last = depth;
+    const long long blocks = tiles_in_plane * zb;
     const long long waves = (blocks + capacity - 1) / capacity;
     const double eff = double(blocks) / double(waves * capacity) * depth / (depth + 2.0) * double(waves) / (double(waves) + 0.1);
     if (eff > best_eff * 1.0001) {
