@@ -59,6 +59,13 @@ WAVE_SIGNATURES = {
     "paraiso_wave_launch_count": (_int, [_vp, _pi64]),
 }
 
+# the allocation-free CFL reduction (include/paraiso_hydro_noalloc.h), exported by the same library
+PARAISO_ETOOLARGE = -6
+NOALLOC_MAX_CELLS = 134217728
+NOALLOC_SIGNATURES = {
+    "paraiso_hydro_cfl_noalloc": (_int, [_int, _pi64, _pdbl, _dbl, _int, _vp, _dbl, _vp, _vp]),
+}
+
 # the probe library (include/paraiso_hydro_probe.h): tests and bench.py's roofline leg only
 PROBE_PATH = os.path.join(HERE, "libparaiso_hydro_probe.so")
 PROBE_SIGNATURES = {
@@ -89,7 +96,7 @@ def load_library(path=None):
         raise ParaisoError(PARAISO_ECUDA, f"{p} not built; run `python -m paper_1204_4779_b200.build` "
                                           "(there is no CPU fallback)")
     lib = ctypes.CDLL(p)
-    for name, (res, args) in list(SIGNATURES.items()) + list(WAVE_SIGNATURES.items()):
+    for name, (res, args) in list(SIGNATURES.items()) + list(WAVE_SIGNATURES.items()) + list(NOALLOC_SIGNATURES.items()):
         fn = getattr(lib, name)  # AttributeError if a declared symbol is not exported
         fn.restype = res
         fn.argtypes = args
@@ -178,6 +185,37 @@ def probe_arith(a, b):
     if rc:
         raise ParaisoError(rc, "probe_arith failed")
     return q, r
+
+
+def cfl_noalloc(U, n, extent, gamma, cfl, out, stream=None):
+    """paraiso_hydro_cfl_noalloc: S, dt and the bad-cell count of the conserved state `U` into `out`, for callers that
+    must not trigger a device allocation (a code whose own arena holds all of HBM, a tool that was only lent the
+    state, a loop that cannot afford cudaMalloc's device-wide synchronisation).  Nothing is allocated here either:
+    U   a contiguous torch CUDA tensor (float32 or float64) of shape (dims + 2, [nz,] [ny,] nx) that the caller owns;
+    out a torch CUDA float64 tensor of 3 elements that the caller owns (S, dt, bad cells), written asynchronously on
+        `stream` (a torch.cuda.Stream or raw cudaStream_t; default: the legacy default stream).
+    At most NOALLOC_MAX_CELLS cells (the working memory is a fixed array inside the library); calls on one device
+    share that array and must not overlap on the GPU; make the first call on a device before any stream capture."""
+    lib = load_library()
+    pu, dt, size = _pointer(U)
+    po, dto, sizeo = _pointer(out)
+    if not (getattr(U, "is_cuda", False) and getattr(out, "is_cuda", False)):
+        raise ValueError("cfl_noalloc wants device tensors for U and out (it copies nothing)")
+    dims = len(n)
+    if dto != np.dtype(np.float64) or sizeo < 3:
+        raise ValueError("out must hold 3 float64 values")
+    if size != (dims + 2) * int(np.prod([int(v) for v in n], dtype=object)):
+        raise ValueError("U does not have (dims + 2) * prod(n) elements")
+    narr = (_i64 * dims)(*[int(v) for v in n])
+    earr = (_dbl * dims)(*[float(e) for e in extent])
+    s = getattr(stream, "cuda_stream", stream)
+    rc = lib.paraiso_hydro_cfl_noalloc(dims, narr, earr, float(gamma), PARAISO_F32 if dt == np.dtype(np.float32) else
+                                       PARAISO_F64, _vp(pu), float(cfl), _vp(int(s) if s else 0), _vp(po))
+    if rc == PARAISO_ETOOLARGE:
+        raise ParaisoError(rc, f"cfl_noalloc: more than {NOALLOC_MAX_CELLS} cells; the built-in scratch cannot hold "
+                               "their per-block partials (use a handle, or reduce sub-boxes and take the larger S)")
+    if rc != PARAISO_OK:
+        raise ParaisoError(rc, "cfl_noalloc failed (bad argument)" if rc == PARAISO_EINVAL else "cfl_noalloc: CUDA error")
 
 
 class ParaisoHydro:
