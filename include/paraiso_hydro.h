@@ -84,7 +84,9 @@ int paraiso_hydro_destroy(paraiso_hydro_t *h);
  *               14 [two halo warps, default on large grids]; fp32 also 5, 11, 15); k_fused: block_x x block_y = tile;
  *               k_march: block_x = main warps per row (2-D), block_y = main warps (3-D), block_z = rows per main
  *               thread (3-D: 1 or 2), cells_per_thread 2 = packed f32x2; tile_depth = planes marched per block
- *               (0: chosen from the kernel's occupancy so that the grid fills whole waves)
+ *               (0: chosen from the kernel's occupancy so that the grid fills whole waves).  A knob the selected
+ *               kernel does not read in this dimension (k_pack / k_march: block_y in 2-D, block_x in 3-D, ...) must be
+ *               0, and staging / arith are honoured in the default tile of k_march only: anything else is EINVAL
  *   "limiter"   interpolation variant (R22): 0 the paper's MINBEE, Eq. 21 (default) | 1 none: piecewise
  *               constant states, the first-order Godunov scheme | 2 monotonized central (van Leer 1977).  1 and 2 are
  *               compile-time variants of k_pack (default launch shape only) and k_delayed; any other kernel -> EINVAL
@@ -93,7 +95,7 @@ int paraiso_hydro_destroy(paraiso_hydro_t *h);
  *               1 hardware reciprocal / reciprocal-square-root approximations: inside north_star's fp32 tolerances,
  *               not bit-equal, ~15 % faster (R21)
  *   "staging"   k_march only: 0 / 1 every thread loads its own cells (default) | 2 TMA bulk copies of the tile rows into a
- *               shared-memory ring (cp.async.bulk; one cell per thread, n_x a multiple of 16 bytes) | 3 the same ring
+ *               shared-memory ring (cp.async.bulk; one cell per thread, n_x a multiple of 16 bytes, else EINVAL) | 3 the same ring
  *               filled by one tensor-map copy per plane (cp.async.bulk.tensor); both measured, DESIGN.md §7
  *   "integrator" 0 the paper's two-stage midpoint rule, Eq. 24-27 (default) | 1 Heun / Shu-Osher SSP-RK2, the
  *               "2-stage TVD Runge-Kutta" north_star names as the fallback (R20): same kernels and traffic

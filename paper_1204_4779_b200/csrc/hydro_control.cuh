@@ -123,6 +123,20 @@ __device__ __forceinline__ void block_reduce_and_finalize(Real s, int bad, Scala
   }
 }
 
+// SMs of the current device (host side; cached per device): what the launch heuristics size their grids against.
+// Falls back to the B200's 148 only if the attribute cannot be read.
+inline int device_sm_count() {
+  static int sms[64] = {};
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return 148;
+  if (!sms[dev]) {
+    int v = 0;
+    if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || v < 1) return 148;
+    sms[dev] = v;
+  }
+  return sms[dev];
+}
+
 enum { CTRL_MANUAL_DT = 0, CTRL_BEGIN_RUN = 1, CTRL_RESET = 2 };
 
 // <<<1,1>>> host-driven control.

@@ -345,7 +345,7 @@ static bool launch_fused_shape(const Real* Uin, const Real* Ubase, Real* Uout, c
 // face per tile stay below ~10 % of the work, shallow enough to give every SM several blocks.
 inline int default_tile_depth(long long tiles_in_plane, int nM) {
   int depth = 32;
-  while (depth > 8 && tiles_in_plane * ((nM + depth - 1) / depth) < 4 * 148) depth >>= 1;
+  while (depth > 8 && tiles_in_plane * ((nM + depth - 1) / depth) < 4 * device_sm_count()) depth >>= 1;
   return depth;
 }
 

@@ -757,7 +757,7 @@ static bool launch_march_shape(const scalar_t<T>* Uin, const scalar_t<T>* Ubase,
 // stay below ~10 % of the work, shallow enough to give every SM several blocks.
 inline int march_default_depth(long long tiles_in_plane, int nM) {
   int depth = 128;
-  while (depth > 8 && tiles_in_plane * ((nM + depth - 1) / depth) < 4 * 148) depth >>= 1;
+  while (depth > 8 && tiles_in_plane * ((nM + depth - 1) / depth) < 4 * device_sm_count()) depth >>= 1;
   return depth;
 }
 
@@ -784,6 +784,15 @@ bool launch_march_stage(const Real* Uin, const Real* Ubase, Real* Uout, const Ge
     const int w = packed ? 2 : 1;
     const bool tma = staging == 2 && !packed && g.n[0] % (16 / (int)sizeof(Real)) == 0;
     const bool tma_map = staging == 3 && !packed && g.n[0] % (16 / (int)sizeof(Real)) == 0;  // tensor-map TMA
+    // A knob this kernel cannot honour is "shape not covered" (false), never the plain kernel under the requested name:
+    // TMA staging needs an unpacked row of whole 16-byte units and the default tile; arith = 1 exists in fp32, default
+    // tile, per-thread loads, one cell per thread; a block_* this dimension does not read must be 0.
+    if (staging < 0 || staging > 3 || (staging >= 2 && !(tma || tma_map))) return false;
+    if (arith < 0 || arith > 1 || (arith == 1 && (!can_pack || packed || staging >= 2 || block[2] == 2))) return false;
+    const int shape_knob = D == 2 ? block[0] : block[1];
+    if ((staging >= 2 || arith == 1) && shape_knob > 0 && shape_knob != (D == 2 ? 4 : 7)) return false;
+    if (D == 2 ? (block[1] != 0 || block[2] != 0) : (block[0] != 0 || block[2] < 0 || block[2] > 2)) return false;
+    if (D == 3 && block[2] == 2 && (packed || staging >= 2 || (block[1] > 0 && block[1] != 7))) return false;
     if constexpr (D == 2) {
       int nwx = block[0] > 0 ? block[0] : 4;
       const long long tiles = (g.n[0] + nwx * 32 * w - 1) / (nwx * 32 * w);

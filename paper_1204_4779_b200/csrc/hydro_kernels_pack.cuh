@@ -550,6 +550,8 @@ bool launch_pack_stage(const Real* Uin, const Real* Ubase, Real* Uout, const Geo
     using T = typename std::conditional<F32, f32x2, double>::type;
     constexpr int W = LaneTraits<T>::W;
     if (W == 2 && g.n[0] % 2 != 0) return false;
+    // a block_* knob this dimension does not read must be 0: "shape not covered", not a silently ignored request
+    if (D == 2 ? (block[1] != 0 || block[2] < 0 || block[2] > 1) : (block[0] != 0 || block[2] != 0)) return false;
     if constexpr (D == 2) {
       // 2-D rows: overlapping tiles, no halo warp (block[2] = 1: the halo-warp form of the same kernel).  Default
       // row width: the one of 2 / 4 / 8 warps that leaves the fewest idle lanes (ghost cells + ragged last tile)
@@ -591,7 +593,7 @@ bool launch_pack_stage(const Real* Uin, const Real* Ubase, Real* Uout, const Geo
       const int tw = 32 * W;
       if (ty <= 0) {
         const long long tiles14 = (long long)((g.n[0] + tw - 1) / tw) * ((g.n[1] + 13) / 14);
-        ty = tiles14 * ((g.n[2] + 127) / 128) >= 4 * 148 ? 14 : 7;
+        ty = tiles14 * ((g.n[2] + 127) / 128) >= 4 * device_sm_count() ? 14 : 7;
       }
       const int depth = tile_depth;  // 0: launch_pack_bnd picks it from the kernel's occupancy
       if (ty == 7) return launch_pack_shape<T, D, RS, STAGE, 1, 7, 2>(Uin, Ubase, Uout, g, sc, stream, depth);

@@ -10,6 +10,7 @@
 namespace ph {
 
 constexpr int SMALL1D_MAX = 1024;
+constexpr long long SMALL1D_MAX_STEPS = 4096;  // steps per launch; the host loops over longer runs
 
 template <class Real, int RS, int LIM>
 __global__ void __launch_bounds__(SMALL1D_MAX) k_small1d(Real* U, Geom<Real> g, Scalars* sc, long long nsteps) {

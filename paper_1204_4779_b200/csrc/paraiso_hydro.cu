@@ -391,13 +391,18 @@ struct Launch {
       const Geom<Real> g = make_geom<Real>(h);
       const int bs = int((h->N + 31) / 32 * 32);
       Real* U = (Real*)h->U[0];
-      if (h->limiter == LIMITER_NONE)
-        k_small1d<Real, RS, LIMITER_NONE><<<1, bs, 0, h->stream>>>(U, g, h->sc, (long long)nsteps);
-      else if (h->limiter == LIMITER_MC)
-        k_small1d<Real, RS, LIMITER_MC><<<1, bs, 0, h->stream>>>(U, g, h->sc, (long long)nsteps);
-      else
-        k_small1d<Real, RS, LIMITER_MINBEE><<<1, bs, 0, h->stream>>>(U, g, h->sc, (long long)nsteps);
-      h->launches += 1;
+      // at most SMALL1D_MAX_STEPS steps per launch: a launch cannot be interrupted, and the kernel carries the whole
+      // time-step control in and out through *sc, so consecutive launches continue exactly where the last one stopped
+      for (int64_t left = nsteps; left > 0; left -= SMALL1D_MAX_STEPS) {
+        const long long k = (long long)(left < SMALL1D_MAX_STEPS ? left : SMALL1D_MAX_STEPS);
+        if (h->limiter == LIMITER_NONE)
+          k_small1d<Real, RS, LIMITER_NONE><<<1, bs, 0, h->stream>>>(U, g, h->sc, k);
+        else if (h->limiter == LIMITER_MC)
+          k_small1d<Real, RS, LIMITER_MC><<<1, bs, 0, h->stream>>>(U, g, h->sc, k);
+        else
+          k_small1d<Real, RS, LIMITER_MINBEE><<<1, bs, 0, h->stream>>>(U, g, h->sc, k);
+        h->launches += 1;
+      }
       h->kernel_used = KERNEL_SMALL1D;
     }
   }
@@ -406,7 +411,7 @@ struct Launch {
     const Geom<Real> g = make_geom<Real>(h);
     const int bs = 256;
     int64_t blocks = (h->N + bs - 1) / bs;
-    if (blocks > 148 * 8) blocks = 148 * 8;
+    if (blocks > device_sm_count() * 8) blocks = device_sm_count() * 8;
     k_cfl<Real, D><<<(unsigned int)blocks, bs, 0, h->stream>>>((const Real*)h->U[0], g, h->sc);
     h->launches += 1;
   }

@@ -157,6 +157,27 @@ def random_smooth(n, dtype=np.float64, seed=0, gamma=1.4, boundary="periodic", j
                     10, 0.0, np.ascontiguousarray(U.astype(dtype)))
 
 
+def hypersonic(n, dtype=np.float32, mach=50.0, seed=3):
+    """Edge-case state (not a BASELINE config): a slab 0.25 < x < 0.75 of (rho, p) = (1, 1) gas in a medium of
+    (1e-6, 1e-6), 1 % noise on both, v_x = +mach c for x < 0.5 and -mach c beyond (c = sqrt(gamma)): supersonic faces of
+    both signs, a 10^6 density jump swept at Mach `mach`, a head-on collision in the middle.  Transverse velocities are
+    0.3 Uniform(-1, 1).  gamma 1.4, periodic, CFL 0.4."""
+    n = tuple(int(v) for v in n)
+    dims = len(n)
+    shape = tuple(reversed(n))
+    rng = np.random.default_rng(seed)
+    gamma = 1.4
+    X = np.broadcast_to(_centres(n[0]), shape)
+    dense = (X > 0.25) & (X < 0.75)
+    rho = np.where(dense, 1.0, 1e-6) * (1.0 + 0.01 * rng.uniform(-1, 1, shape))
+    p = np.where(dense, 1.0, 1e-6) * (1.0 + 0.01 * rng.uniform(-1, 1, shape))
+    c = np.sqrt(gamma)
+    v = [np.where(X < 0.5, mach * c, -mach * c) * np.ones(shape)] + [0.3 * rng.uniform(-1, 1, shape) for _ in range(dims - 1)]
+    U = conserved_from_primitive(rho, v, p, gamma)
+    return Workload(f"hypersonic{dims}d_{'x'.join(map(str, n))}_mach{mach:g}", n, tuple(1.0 for _ in n), gamma,
+                    np.dtype(dtype), "periodic", 0.4, 3, 0.0, np.ascontiguousarray(U.astype(dtype)))
+
+
 def baseline_config(i, scale=1.0):
     """BASELINE.json configs[i]; scale < 1 shrinks the grid (same recipe) for quick parity runs."""
     s = lambda m: max(8, int(round(m * scale)))

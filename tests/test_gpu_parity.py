@@ -96,6 +96,7 @@ def test_hundred_steps_match_oracle(gpu, oracle_mod, variant, dims, dtype):
     assert abs(gdt[-1] - rdt[-1]) <= max(told, tol100 * 1e-1) * rdt[-1]
     err = field_errors(got, ref)
     assert np.all(err <= tol100), (variant, err)
+    assert np.array_equal(got, ref), (variant, "100 steps of the same written arithmetic: bit-equal")
 
 
 @pytest.mark.parametrize("variant", VARIANTS)
@@ -315,6 +316,32 @@ def test_uncovered_shapes_are_errors(gpu, oracle_mod):
             assert ei.value.code == gpu.PARAISO_EINVAL and "not covered" in str(ei.value), (variant, opts)
             with pytest.raises(gpu.ParaisoError):
                 h.run(0.4, 16)  # the same inside a graph capture
+    # a knob the requested kernel cannot honour is an error too, not the plain kernel under the requested name:
+    # TMA staging / arith = 1 outside the default tile, arith = 1 in fp64, staging on a row that is not whole 16-byte
+    # units, and block_* knobs the kernel does not read in this dimension
+    w3 = inputs.random_smooth((152, 36), np.float32, seed=5)
+    w3d = inputs.random_smooth((152, 36), np.float64, seed=5)
+    w4 = inputs.random_smooth((64, 24, 9), np.float32, seed=6)
+    strict = [(w, "march", {"staging": 2}), (w, "march", {"staging": 3}),
+              (w3, "march", {"block_x": 2, "staging": 2}), (w3, "march", {"block_x": 2, "arith": 1}),
+              (w3, "march", {"staging": 2, "arith": 1}), (w3, "march", {"block_y": 4}), (w3, "march", {"block_z": 2}),
+              (w3, "pack", {"block_y": 7}), (w3, "pack", {"block_z": 2}), (w3, "fused", {"block_y": 7}),
+              (w3d, "march", {"arith": 1}), (w3d, "fused", {"arith": 1}),
+              (w4, "march", {"block_x": 2}), (w4, "pack", {"block_x": 2}), (w4, "pack", {"block_z": 1}),
+              (w4, "march", {"block_y": 4, "staging": 3}), (w4, "march", {"block_y": 4, "arith": 1}),
+              (w4, "march", {"block_y": 8, "block_z": 2}), (w4, "march", {"block_z": 2, "arith": 1})]
+    for wk, variant, opts in strict:
+        with gpu.ParaisoHydro(wk.n, wk.extent, wk.gamma, wk.dtype, wk.boundary, "hllc", variant, **opts) as h:
+            h.set_state(wk.U)
+            with pytest.raises(gpu.ParaisoError) as ei:
+                h.step(1e-4)
+            assert ei.value.code == gpu.PARAISO_EINVAL and "not covered" in str(ei.value), (wk.n, variant, opts)
+    for wk, opts in ((w3, {"staging": 2}), (w3, {"staging": 3}), (w3, {"arith": 1}), (w3, {"block_x": 4, "arith": 1}),
+                     (w4, {"block_y": 7, "staging": 2}), (w4, {"block_z": 2}), (w4, {"block_y": 7, "block_z": 2})):
+        with gpu.ParaisoHydro(wk.n, wk.extent, wk.gamma, wk.dtype, wk.boundary, "hllc", "march", **opts) as h:
+            h.set_state(wk.U)
+            h.step(1e-4)  # honoured knobs still run
+            assert h.get_option("kernel_used") == KERNEL_ID["march"], opts
     w1 = inputs.sod(64)
     for variant in ("march", "fused1", "pack"):
         with gpu.ParaisoHydro(w1.n, w1.extent, w1.gamma, w1.dtype, "outflow", "hllc", variant) as h:
@@ -428,11 +455,33 @@ def test_heun_integrator_option_matches_oracle(gpu, oracle_mod, variant, dims, d
     assert np.array_equal(got, ref)
 
 
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("n", [(64, 24), (64, 12, 6), (256,)])
+def test_hypersonic_flow_into_near_vacuum_matches_oracle(gpu, oracle_mod, n, dtype):
+    """Mach-50 streams of (rho, p) = (1, 1) gas running from both sides into a medium a million times thinner and
+    colliding head-on (inputs.hypersonic): almost every x face is supersonic, with S_K - S* as small as it gets beside
+    v ~ 60.  This is where the packed HLLC's shortcut for supersonic faces, F = fma(0, U* - U_K, F_K) (hydro_math.cuh;
+    exact only while U* is finite), could part from the oracle, which never forms U* on that branch.
+    Bit-equal after 1 and 3 steps for every on-chip kernel and both solvers, and no cell is flagged."""
+    w = inputs.hypersonic(n, dtype)
+    for riemann in ("hllc", "hll"):
+        for nsteps in (1, 3):
+            ref, rdt = oracle_steps(oracle_mod, w, nsteps, riemann=riemann)
+            assert np.isfinite(ref).all() and (ref[0] > 0).all()
+            for variant in ("fused", "pack", "march", "delayed"):
+                if not covers(variant, len(n), dtype, n):
+                    continue
+                got, gdt = gpu_steps(gpu, w, nsteps, variant, riemann=riemann)  # asserts stats() == 0
+                assert np.array_equal(got, ref), (variant, riemann, nsteps, field_errors(got, ref))
+                assert all(abs(a - b) <= TOL[np.dtype(dtype)][2] * b for a, b in zip(gdt, rdt))
+
+
 @pytest.mark.parametrize("boundary", ["periodic", "outflow"])
 @pytest.mark.parametrize("dims,shape", [(2, (256, 45)), (2, (300, 33)), (3, (64, 30, 21)), (3, (96, 13, 150)), (3, (40, 9, 9))])
 def test_march_tma_staging_matches_oracle(gpu, oracle_mod, dims, shape, boundary):
     """staging = 2: the tile rows of U_in / U_base arrive by TMA bulk copies in a shared-memory ring (tiles that end
-    inside the grid; ragged tiles and n_x not a multiple of 16 bytes take the per-thread loads)."""
+    inside the grid; ragged tiles inside the kernel take the per-thread loads; a grid whose n_x is not a multiple of
+    16 bytes is "shape not covered": test_uncovered_shapes_are_errors)."""
     for dtype in (np.float32, np.float64):
         w = inputs.random_smooth(shape, dtype, seed=41 + dims, boundary=boundary)
         ref, rdt = oracle_steps(oracle_mod, w, 3)
@@ -610,3 +659,24 @@ def test_small_1d_grids_run_in_one_launch(gpu, oracle_mod, n, dtype):
         h.set_state(w.U)
         h.run(w.cfl, 3)
         assert h.get_option("kernel_used") == KERNEL_ID["delayed"]
+
+
+def test_small_1d_long_runs_are_split_into_bounded_launches(gpu, oracle_mod):
+    """k_small1d advances at most 4096 steps per launch (a launch cannot be interrupted); the host loops, and the
+    device-side time-step control carries over between launches: 9000 steps = 3 launches, bit-equal to the oracle."""
+    w = inputs.random_smooth((64,), np.float64, seed=12)
+    o = oracle_mod.Oracle(w.n, w.extent, w.gamma, w.dtype, "periodic", "hllc", "serial", "midpoint")
+    o.set_state(w.U)
+    k, t = o.run(w.cfl, 9000)
+    ref = o.get_state()
+    o.close()
+    with gpu.ParaisoHydro(w.n, w.extent, w.gamma, w.dtype) as h:
+        h.set_state(w.U)
+        l0 = h.launch_count()
+        h.run(w.cfl, 9000)
+        got = h.get_state()
+        assert h.launch_count() - l0 == 1 + 3  # the control kernel + ceil(9000 / 4096) stage kernels
+        assert h.get_option("kernel_used") == KERNEL_ID["small1d"]
+        tg, kg = h.time()
+        assert kg == k == 9000 and abs(tg - t) <= 1e-9 * t and h.stats() == 0
+    assert np.array_equal(got, ref)
