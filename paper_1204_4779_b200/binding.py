@@ -225,6 +225,8 @@ class ParaisoHydro:
                  **options):
         self._lib = load_library()
         self._h = _vp()
+        self._stream_ptr = 0          # the handle's stream (0 = legacy default), mirrored for _source()
+        self._pending_sources = []    # sources of asynchronous copies, released at the next blocking call
         self.n = tuple(int(v) for v in n)
         self.dims = len(self.n)
         self.nf = self.dims + 2
@@ -275,9 +277,36 @@ class ParaisoHydro:
         """stream: a raw cudaStream_t integer or a torch.cuda.Stream."""
         s = getattr(stream, "cuda_stream", stream)
         self._check(self._lib.paraiso_hydro_set_stream(self._h, _vp(int(s) if s else 0)))
+        self._stream_ptr = int(s) if s else 0
+
+    def _source(self, a):
+        """Pointer of an array the library will read ASYNCHRONOUSLY on the handle's stream (set_state, set_ghosts,
+        step_ghosts with a device or pinned source).  Two things the C ABI leaves to the caller are done here: the
+        source object is kept alive until the handle's next blocking call (a temporary such as
+        `h.set_state(torch.from_numpy(U).cuda())` would otherwise go back to torch's caching allocator and could be
+        reused before the copy has run), and a torch CUDA source, which torch produced on ITS current stream, is
+        ordered before the handle's stream by an event when the two streams differ."""
+        ptr = self._state_ptr(a)
+        if len(self._pending_sources) >= 64:  # a long loop of asynchronous calls: drain instead of hoarding
+            self.sync()
+        self._pending_sources.append(a)
+        if getattr(a, "is_cuda", False):
+            import torch
+
+            cur = torch.cuda.current_stream(a.device)
+            if int(cur.cuda_stream) != self._stream_ptr:
+                mine = (torch.cuda.ExternalStream(self._stream_ptr, device=a.device) if self._stream_ptr
+                        else torch.cuda.default_stream(a.device))
+                ev = torch.cuda.Event()
+                ev.record(cur)
+                mine.wait_event(ev)
+        return ptr
+
+    def _blocking_call_done(self):
+        self._pending_sources.clear()
 
     def set_state(self, U):
-        self._check(self._lib.paraiso_hydro_set_state(self._h, _vp(self._state_ptr(U))))
+        self._check(self._lib.paraiso_hydro_set_state(self._h, _vp(self._source(U))))
 
     def get_state(self, out=None):
         if out is None:
@@ -288,6 +317,7 @@ class ParaisoHydro:
     def cfl_dt(self, cfl):
         dt = _dbl(0)
         self._check(self._lib.paraiso_hydro_cfl_dt(self._h, float(cfl), ctypes.byref(dt)))
+        self._blocking_call_done()
         return dt.value
 
     def step(self, dt):
@@ -296,11 +326,11 @@ class ParaisoHydro:
     def set_ghosts(self, G):
         """Prescribed ghost cells (include/paraiso_hydro.h): the outermost two cells of every axis of the current
         state := G's.  G: array / tensor shaped like the state (host or device)."""
-        self._check(self._lib.paraiso_hydro_set_ghosts(self._h, self._state_ptr(G)))
+        self._check(self._lib.paraiso_hydro_set_ghosts(self._h, self._source(G)))
 
     def step_ghosts(self, dt, G_mid):
         """One RK2 step whose intermediate state gets G_mid's ghost cells before the second stage."""
-        self._check(self._lib.paraiso_hydro_step_ghosts(self._h, float(dt), self._state_ptr(G_mid)))
+        self._check(self._lib.paraiso_hydro_step_ghosts(self._h, float(dt), self._source(G_mid)))
 
     def run(self, cfl, nsteps, t_end=0.0):
         k, t = _i64(0), _dbl(0)
@@ -310,6 +340,7 @@ class ParaisoHydro:
 
     def sync(self):
         self._check(self._lib.paraiso_hydro_sync(self._h))
+        self._blocking_call_done()
 
     def time(self):
         t, k = _dbl(0), _i64(0)
@@ -342,8 +373,9 @@ class ParaisoHydro:
 
     def destroy(self):
         if getattr(self, "_h", None) and self._h.value:
-            self._lib.paraiso_hydro_destroy(self._h)
+            self._lib.paraiso_hydro_destroy(self._h)  # synchronises the device
             self._h = _vp()
+            self._pending_sources.clear()
 
     close = destroy
 
