@@ -289,11 +289,18 @@ def e2e_run(binding, torch, w, steps, warmup, variant, riemann):
 # kernels execute (fp32: 1 MUFU + 5 / 4 operations, fp64: 1 MUFU + 7 / 9).  Roofline (b) of north_star = these
 # operations over the FP32 (128 lanes per SM) or FP64 (64 lanes per SM) lane rate of 148 SMs at 1.965 GHz.
 COUNTED_OPS_PER_CELL_STEP = {(1, 4): 299, (2, 4): 638, (3, 4): 1053, (1, 8): 354, (2, 8): 737, (3, 8): 1196}
-SM_COUNT, SM_MAX_GHZ = 148, 1.965
+SM_MAX_GHZ = 1.965
+
+
+def sm_count():
+    """SMs of the device in use (148 on a B200), from the driver."""
+    import torch
+
+    return int(torch.cuda.get_device_properties(torch.cuda.current_device()).multi_processor_count)
 
 
 def alu_peak_tlaneops(itemsize):
-    return SM_COUNT * (128 if itemsize == 4 else 64) * SM_MAX_GHZ * 1e9 / 1e12
+    return sm_count() * (128 if itemsize == 4 else 64) * SM_MAX_GHZ * 1e9 / 1e12
 
 
 # arith = 1 (f32fast): an IEEE division (1 MUFU + 5) / square root (1 MUFU + 4) becomes 1 MUFU + 1 multiplication
@@ -328,17 +335,21 @@ def roofline_of(w, r, peak, peak_src, traffic=None, binding=None, counted_ops=No
     alu_achieved = ops / (avg_ms * 1e-3) / 1e12
     alu_nominal = alu_peak_tlaneops(isz)
     alu_measured = measured_alu_peak(binding, isz) if binding is not None else None
-    alu_peak = alu_measured or alu_nominal
+    # `frac` divides by the FIXED nominal peak (unit counts x max clock) so that rounds stay comparable; the peak the
+    # probe measured on this device in this run (best of 5 short launches: it moves with the power state) is reported
+    # beside it as peak_measured / frac_of_measured.  DESIGN.md §8: north_star's 0.70 is read against `frac`.
+    alu_peak = alu_nominal
     hbm = {"bound": "hbm", "achieved": hbm_achieved, "peak": peak, "unit": "GB/s", "frac": hbm_achieved / peak,
            "algorithmic_bytes_per_launch": nbytes, "peak_source": peak_src,
            "gcell_per_s_at_peak": peak * 1e9 / (4 * w.nf * isz) / 1e9}
     alu = {"bound": "alu", "achieved": alu_achieved, "peak": alu_peak, "unit": "Tlaneop/s", "frac": alu_achieved / alu_peak,
            "algorithmic_ops_per_launch": ops, "counted_ops_per_cell_step": counted,
-           "peak_source": ("measured: %s fused multiply-adds per second on this device (paraiso_probe_peak)"
-                           % ("max(FFMA, FFMA2)" if isz == 4 else "DFMA")) if alu_measured else "nominal (no probe library)",
+           "peak_source": "nominal: %d SMs x %d %s lanes x %.3f GHz (B200_PROFILING.md unit counts and clocks.max.sm)"
+                          % (sm_count(), 128 if isz == 4 else 64, "FP32" if isz == 4 else "FP64", SM_MAX_GHZ),
            "peak_nominal": alu_nominal, "frac_of_nominal": alu_achieved / alu_nominal,
-           "peak_nominal_source": "148 SMs x %d %s lanes x 1.965 GHz (B200_PROFILING.md unit counts and clocks.max.sm)"
-                                  % (128 if isz == 4 else 64, "FP32" if isz == 4 else "FP64"),
+           "peak_measured": alu_measured, "frac_of_measured": (alu_achieved / alu_measured) if alu_measured else None,
+           "peak_measured_source": ("%s fused multiply-adds per second on this device (paraiso_probe_peak)"
+                                    % ("max(FFMA, FFMA2)" if isz == 4 else "DFMA")) if alu_measured else None,
            "gcell_per_s_at_peak": alu_peak * 1e12 / counted / 1e9}
     first, other = (alu, hbm) if alu["gcell_per_s_at_peak"] < hbm["gcell_per_s_at_peak"] else (hbm, alu)
     out = dict(first)
