@@ -37,8 +37,8 @@ def gpu():
     return binding
 
 
-def oracle_run(oracle_mod, w, nsteps):
-    o = oracle_mod.Oracle(w.n, w.extent, w.gamma, w.dtype, w.boundary, "hllc", "omp")
+def oracle_run(oracle_mod, w, nsteps, riemann="hllc"):
+    o = oracle_mod.Oracle(w.n, w.extent, w.gamma, w.dtype, w.boundary, riemann, "omp")
     o.set_state(w.U)
     first = None
     t = 0.0
@@ -53,28 +53,34 @@ def oracle_run(oracle_mod, w, nsteps):
     return first, out, t
 
 
-@pytest.mark.parametrize("cfg", [1, 2, 3])
-def test_full_config_matches_oracle(gpu, oracle_mod, cfg):
+@pytest.mark.parametrize("cfg,riemann", [(1, "hllc"), (2, "hllc"), (3, "hllc"), (1, "hll"), (3, "hll")])
+def test_full_config_matches_oracle(gpu, oracle_mod, cfg, riemann):
+    """Configs 1-3 at their stated size and length, HLLC (the paper's solver) and HLL (north_star's fallback; SURVEY A4:
+    "parity is required for both"): every conserved field on its own scale max|ref_f| inside north_star's tolerance
+    (config 1's m_y, ~0.02 beside m_x ~ 1, is the tight one), and - since the kernels state the oracle's arithmetic
+    operation by operation - bit-equal after the first step and after the last."""
     import torch
 
     w = inputs.baseline_config(cfg)
-    (ref1, rdt1), ref, rt = oracle_run(oracle_mod, w, w.steps)
+    (ref1, rdt1), ref, rt = oracle_run(oracle_mod, w, w.steps, riemann)
     tol1, tol100, toldt = TOL[np.dtype(w.dtype)]
-    with gpu.ParaisoHydro(w.n, w.extent, w.gamma, w.dtype, w.boundary, "hllc") as h:
+    with gpu.ParaisoHydro(w.n, w.extent, w.gamma, w.dtype, w.boundary, riemann) as h:
         h.set_state(torch.from_numpy(w.U).cuda())
         gdt1 = h.cfl_dt(w.cfl)
         assert abs(gdt1 - rdt1) <= toldt * rdt1
         h.run(w.cfl, 1)
         got1 = h.get_state()
-        assert np.all(field_errors(got1, ref1) <= tol1), field_errors(got1, ref1)
+        assert np.all(own_scale_errors(got1, ref1) <= tol1), own_scale_errors(got1, ref1)
+        assert np.array_equal(got1, ref1), (cfg, riemann, "first step: bit-equal")
         h.run(w.cfl, w.steps - 1)
         got = h.get_state()
         t, k = h.time()
         assert h.stats() == 0 and k == w.steps
     assert abs(t - rt) <= 10 * toldt * rt, (t, rt)
-    err = field_errors(got, ref)
-    assert np.all(err <= tol100), (cfg, err)
-    print(f"config {cfg}: {w.steps} steps, max field error {err.max():.2e}, bit-equal {np.array_equal(got, ref)}")
+    err = own_scale_errors(got, ref)
+    assert np.all(err <= tol100), (cfg, riemann, err)
+    assert np.array_equal(got, ref), (cfg, riemann, f"after {w.steps} steps: bit-equal")
+    print(f"config {cfg} {riemann}: {w.steps} steps, max own-scale field error {err.max():.2e}, bit-equal True")
 
 
 def wrapped_box(U, lo, size):
