@@ -13,9 +13,9 @@ are added to the same JSON line under "all_configs" (short runs; config 1 is L2-
             get_state(host) every step, copies inside the timed region
   roofline  dominant kernel = the RK stage kernel, duration = CUDA events around every stage launch inside the timed
             region.  north_star's roofline is the slower of (a) 2*nf*w*N algorithmic bytes per launch over the measured
-            copy bandwidth (MEASURED_PEAKS.json) and (b) the counted arithmetic of DESIGN.md §8 over the FP32 / FP64
-            lane rate; the binding one is reported as `bound`, the other under `other_bound`; `traffic` = ncu DRAM
-            bytes per launch (profiles/traffic.csv); `issue_cost_cycles` = measured issue cost per instruction class
+            copy bandwidth (MEASURED_PEAKS.json) and (b) the counted arithmetic of DESIGN.md §8 over the NOMINAL FP32 / FP64
+            lane rate (`counted_ops_oracle`: the same run against the oracle's mechanical count, profiles/r3_counted_ops.json); the binding one is reported as `bound`, the other under `other_bound`; `traffic` = ncu DRAM
+            bytes per launch (profiles/r*_cfg*_ncu_raw.csv); `issue_cost_cycles` = measured issue cost per instruction class
   cpu_baseline  the oracle as it stands, single-threaded and OpenMP, on a bounded sample of the same workload
 
 N > 1: replicas only (DESIGN.md §9): every rank advances its own copy of the workload, no data-path collective;
@@ -321,7 +321,28 @@ def measured_alu_peak(binding, itemsize):
     return _MEASURED_ALU_PEAK[itemsize]
 
 
-def roofline_of(w, r, peak, peak_src, traffic=None, binding=None, counted_ops=None):
+_ORACLE_COUNTS = None
+
+
+def oracle_counted_ops(dims, itemsize, riemann):
+    """The mechanical count of profiles/r3_counted_ops.json (the oracle instantiated with a counting scalar type,
+    `python -m oracle.count_ops`; a committed table, nothing under oracle/ is executed here): issue slots per cell per
+    RK2 step for this dimension / precision / solver as {"composed": ..., "as_written": ...}, or None."""
+    global _ORACLE_COUNTS
+    if _ORACLE_COUNTS is None:
+        _ORACLE_COUNTS = {}
+        try:
+            for row in json.load(open(os.path.join(ROOT, "profiles", "r3_counted_ops.json")))["rows"]:
+                a = row["after_20_steps"]
+                _ORACLE_COUNTS.setdefault((row["dims"], row["itemsize"], row["riemann"]),
+                                          {"composed": a["composed"]["slots"], "as_written": a["as_written"]["slots"],
+                                           "workload": row["workload"]})
+        except Exception:
+            pass
+    return _ORACLE_COUNTS.get((dims, itemsize, riemann))
+
+
+def roofline_of(w, r, peak, peak_src, traffic=None, binding=None, counted_ops=None, riemann="hllc"):
     """The slower of north_star's two rooflines is the binding one and is reported as `bound`; the other is kept
     beside it.  (a) HBM: 2*nf*w*N algorithmic bytes per stage launch (state read once, written once; halo excluded)
     over the measured copy bandwidth.  (b) ALU: counted lane-operations per stage launch over the FP32 / FP64 lane
@@ -330,7 +351,15 @@ def roofline_of(w, r, peak, peak_src, traffic=None, binding=None, counted_ops=No
     nbytes = 2 * w.nf * isz * w.cells
     avg_ms = r["stage_ms"] / max(1, r["stage_launches"])
     hbm_achieved = nbytes / (avg_ms * 1e-3) / 1e9
-    counted = counted_ops or COUNTED_OPS_PER_CELL_STEP[(w.dims, isz)]
+    # numerator: HLLC = the hand table of what the kernels execute (upwind side chosen first, selects counted); HLL has
+    # no hand table: the oracle's mechanical count (composed: one interpolation per cell and axis) stands in for it
+    mech = oracle_counted_ops(w.dims, isz, riemann)
+    if counted_ops:
+        counted, count_src = counted_ops, "hand table, arith = 1 (DESIGN.md R21)"
+    elif riemann == "hll" and mech:
+        counted, count_src = mech["composed"], "profiles/r3_counted_ops.json: oracle with a counting scalar, composed, HLL"
+    else:
+        counted, count_src = COUNTED_OPS_PER_CELL_STEP[(w.dims, isz)], "hand table of DESIGN.md §8 (HLLC, what the kernels execute)"
     ops = counted / 2.0 * w.cells
     alu_achieved = ops / (avg_ms * 1e-3) / 1e12
     alu_nominal = alu_peak_tlaneops(isz)
@@ -343,7 +372,13 @@ def roofline_of(w, r, peak, peak_src, traffic=None, binding=None, counted_ops=No
            "algorithmic_bytes_per_launch": nbytes, "peak_source": peak_src,
            "gcell_per_s_at_peak": peak * 1e9 / (4 * w.nf * isz) / 1e9}
     alu = {"bound": "alu", "achieved": alu_achieved, "peak": alu_peak, "unit": "Tlaneop/s", "frac": alu_achieved / alu_peak,
-           "algorithmic_ops_per_launch": ops, "counted_ops_per_cell_step": counted,
+           "algorithmic_ops_per_launch": ops, "counted_ops_per_cell_step": counted, "counted_ops_source": count_src,
+           # the same run read against the oracle's mechanical counts; nominal peak
+           "counted_ops_oracle": None if not mech else {
+               "composed": mech["composed"], "as_written": mech["as_written"],
+               "frac_composed": mech["composed"] / 2.0 * w.cells / (avg_ms * 1e-3) / 1e12 / alu_nominal,
+               "frac_as_written": mech["as_written"] / 2.0 * w.cells / (avg_ms * 1e-3) / 1e12 / alu_nominal,
+               "source": "profiles/r3_counted_ops.json (python -m oracle.count_ops), %s, %s" % (mech["workload"], riemann)},
            "peak_source": "nominal: %d SMs x %d %s lanes x %.3f GHz (B200_PROFILING.md unit counts and clocks.max.sm)"
                           % (sm_count(), 128 if isz == 4 else 64, "FP32" if isz == 4 else "FP64", SM_MAX_GHZ),
            "peak_nominal": alu_nominal, "frac_of_nominal": alu_achieved / alu_nominal,
@@ -474,7 +509,7 @@ def main():
                        "variant": args.variant, "options": options, "parallelism": "replicas" if world > 1 else "1gpu",
                        "l2": "state buffers (2 x %.0f MB) exceed the 126 MB L2; no flush needed" % (w.U.nbytes / 1e6)
                        if 2 * w.U.nbytes > 126e6 else "L2-RESIDENT workload (2 x %.1f MB): not an HBM number" % (w.U.nbytes / 1e6)},
-            "roofline": roofline_of(w, r, peak, peak_src, binding=binding if rank == 0 else None,
+            "roofline": roofline_of(w, r, peak, peak_src, binding=binding if rank == 0 else None, riemann=args.riemann,
                                     counted_ops=COUNTED_OPS_ARITH1.get((w.dims, w.dtype.itemsize)) if options.get("arith") == 1 else None),
             "e2e": e2e, "gpu_launches": r["launches"], "clocks": clocks}
     traffic, traffic_file = ncu_traffic(args.config, args.variant) if not options else (None, None)
@@ -499,6 +534,13 @@ def main():
         line["all_configs"] = sweep(binding, torch, args, peak, peak_src)
     if rank == 0 and not args.no_cpu:
         line["cpu_baseline"] = cpu_baseline(w)
+    if rank == 0 and "all_configs" in line:
+        # LAST key on purpose (a reader of the tail of the line sees every config): the default variant of each config,
+        # HLLC and HLL, with the fraction of the binding roofline (nominal peak) and its own clock sample
+        line["configs_summary"] = [{"config": x["config"], "riemann": x.get("riemann", args.riemann), "gcell_per_s": round(x["value"], 3),
+                                    "bound": x["bound"], "frac": round(x["frac"], 4), "sm_mhz": x["clocks"]["sm_mhz"],
+                                    "reasons": x["clocks"]["reasons"]}
+                                   for x in line["all_configs"] if x.get("variant") == "fused" and "error" not in x]
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()
@@ -516,8 +558,13 @@ def sweep(binding, torch, args, peak, peak_src):
         w = make_workload(cfg)
         big = w.cells >= (1 << 22)
         steps = min(DEFAULT_STEPS[cfg], 100 if not big else 10)
-        for variant in ("fused", "pack", "march", "fused1", "manifest_flux", "manifest_all", "delayed", "march arith=1"):
+        for variant in ("fused", "fused hll", "pack", "march", "fused1", "manifest_flux", "manifest_all", "delayed", "march arith=1"):
             opts, counted = None, None
+            riemann = args.riemann
+            if variant == "fused hll":  # HLL reported beside HLLC for the default variant of configs 1-4
+                if cfg not in (1, 2, 3, 4) or args.riemann == "hll":
+                    continue
+                riemann = "hll"
             if variant == "march arith=1":  # fp32 only: hardware rcp / rsqrt approximations, inside the tolerances, not bit-equal
                 if w.dtype != np.float32 or w.dims == 1:
                     continue
@@ -528,14 +575,15 @@ def sweep(binding, torch, args, peak, peak_src):
             sampler = ClockSampler(local).start()
             t0 = time.time()
             try:
-                r = device_run(binding, torch, w, steps, 3, variant.split()[0], args.riemann, big, opts)
+                r = device_run(binding, torch, w, steps, 3, variant.split()[0], riemann, big, opts)
             except Exception as ex:  # shape not covered, out of memory for manifest_all, ...
                 sampler.stop(t0, time.time())
                 out.append({"config": cfg, "variant": variant, "error": str(ex)[:120]})
                 continue
             clocks = sampler.stop(t0, time.time())
-            rl = roofline_of(w, r, peak, peak_src, binding=binding, counted_ops=counted)
-            out.append({"config": cfg, "workload": w.name, "variant": variant, "steps": steps,
+            rl = roofline_of(w, r, peak, peak_src, binding=binding, counted_ops=counted, riemann=riemann)
+            out.append({"config": cfg, "workload": w.name, "variant": variant.split()[0] if variant == "fused hll" else variant,
+                        "riemann": riemann, "steps": steps,
                         "value": w.cells * steps / (r["ms"] * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": r["ms"] / steps,
                         "bound": rl["bound"], "frac": rl["frac"],
                         "hbm_frac": (rl if rl["bound"] == "hbm" else rl["other_bound"])["frac"],
