@@ -398,15 +398,18 @@ _UNIT_BYTES = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1
 
 def ncu_traffic(cfg, variant):
     """dram__bytes_read.sum + dram__bytes_write.sum per STAGE of the RK2 step, parsed from the committed raw ncu export
-    profiles/r2_cfg<cfg>_<variant>_ncu_raw.csv (`ncu -i ... --page raw --csv` of one `ncu --set full` capture that
+    profiles/r<round>_cfg<cfg>_<variant>_ncu_raw.csv (newest round first) (`ncu -i ... --page raw --csv` of one `ncu --set full` capture that
     holds exactly the kernels of ONE step, the .md beside it names the command): the sum over every captured launch
     divided by the two stages.  For the one-kernel-per-stage variants that is the mean of the two stage launches.
     Returns (bytes per stage, file name) or (None, None) if that configuration was not captured."""
     import csv
 
-    name = f"r2_cfg{cfg}_{variant}_ncu_raw.csv"
-    p = os.path.join(ROOT, "profiles", name)
-    if not os.path.exists(p):
+    for rnd in ("r3", "r2"):  # the newest committed capture of this configuration
+        name = f"{rnd}_cfg{cfg}_{variant}_ncu_raw.csv"
+        p = os.path.join(ROOT, "profiles", name)
+        if os.path.exists(p):
+            break
+    else:
         return None, None
     try:
         rows = list(csv.reader(open(p)))

@@ -405,8 +405,7 @@ class ParaisoWave:
             self._h = _vp()
             raise ParaisoError(rc, "paraiso_wave_create failed (no CUDA device: there is no CPU fallback)" if rc == PARAISO_ECUDA
                                else "paraiso_wave_create failed")
-        self.dx = 2.0 * np.pi / self.n
-        self.dt = self.dx / float(c)
+        self.c = float(c)  # dx = 2 pi / n and dt = dx / c are formed inside the library (include/paraiso_wave.h)
 
     def _check(self, rc):
         if rc != PARAISO_OK:
