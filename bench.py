@@ -326,7 +326,7 @@ _ORACLE_COUNTS = None
 
 def oracle_counted_ops(dims, itemsize, riemann):
     """The mechanical count of profiles/r3_counted_ops.json (the oracle instantiated with a counting scalar type,
-    `python -m oracle.count_ops`; a committed table, nothing under oracle/ is executed here): issue slots per cell per
+    `python tests/count_ops.py`; a committed table, nothing under oracle/ is executed here): issue slots per cell per
     RK2 step for this dimension / precision / solver as {"composed": ..., "as_written": ...}, or None."""
     global _ORACLE_COUNTS
     if _ORACLE_COUNTS is None:
@@ -378,7 +378,7 @@ def roofline_of(w, r, peak, peak_src, traffic=None, binding=None, counted_ops=No
                "composed": mech["composed"], "as_written": mech["as_written"],
                "frac_composed": mech["composed"] / 2.0 * w.cells / (avg_ms * 1e-3) / 1e12 / alu_nominal,
                "frac_as_written": mech["as_written"] / 2.0 * w.cells / (avg_ms * 1e-3) / 1e12 / alu_nominal,
-               "source": "profiles/r3_counted_ops.json (python -m oracle.count_ops), %s, %s" % (mech["workload"], riemann)},
+               "source": "profiles/r3_counted_ops.json (python tests/count_ops.py), %s, %s" % (mech["workload"], riemann)},
            "peak_source": "nominal: %d SMs x %d %s lanes x %.3f GHz (B200_PROFILING.md unit counts and clocks.max.sm)"
                           % (sm_count(), 128 if isz == 4 else 64, "FP32" if isz == 4 else "FP64", SM_MAX_GHZ),
            "peak_nominal": alu_nominal, "frac_of_nominal": alu_achieved / alu_nominal,

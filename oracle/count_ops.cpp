@@ -5,7 +5,7 @@
 // are plain Base values, so every data-dependent branch (MINBEE cases, supersonic faces, the upwind side) is taken
 // exactly as in the fp32 / fp64 run.  Built without OpenMP (the pragmas are ignored; the tallies are plain globals).
 //
-// Two counts come out of it (oracle/count_ops.py turns them into the committed table):
+// Two counts come out of it (tests/count_ops.py turns them into the committed table):
 //   as_written : cfl_S() + step() run whole.  The oracle forms both faces' interpolations per face (every cell is
 //                interpolated twice per axis) and both sides' U_K, F_K before the upwind test, as DESIGN.md §4 writes it.
 //   composed   : the same member functions called piece by piece on the same data and put together as a kernel that

@@ -1,8 +1,9 @@
 """Mechanical operation count of one Euler step: the oracle's Solver instantiated with a counting
 scalar type (oracle/count_ops.cpp) on the BASELINE recipes at reduced size.  TEST / MEASUREMENT INFRASTRUCTURE: calls
-only oracle/ and the seeded input generators; the CUDA path is not involved.
+only oracle/ and the seeded input generators; the CUDA path is not involved.  It sits in tests/ because, like the
+tests, it brings the oracle and the shared input generators together (oracle/ itself imports nothing of the package).
 
-    python -m oracle.count_ops            # prints the table, writes profiles/r3_counted_ops.json and .md
+    python tests/count_ops.py            # prints the table, writes profiles/r3_counted_ops.json and .md
 
 Per config and Riemann solver it reports operations per cell per RK2 step (both stages + the CFL term) by class, for
 the state as generated and for the state 20 oracle steps later (the branch mix - supersonic faces, limiter cases -
@@ -25,8 +26,10 @@ import sys
 
 import numpy as np
 
-HERE = os.path.dirname(os.path.abspath(__file__))
-ROOT = os.path.dirname(HERE)
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+HERE = os.path.join(ROOT, "oracle")  # the counting translation unit and its library live beside the oracle
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
 SRC = os.path.join(HERE, "count_ops.cpp")
 OUT = os.path.join(HERE, "liboracle_count.so")
 CLASSES = ["add", "mul", "fma", "div", "sqrt", "cmp", "minmax", "abs", "neg", "copysign"]
@@ -87,14 +90,14 @@ def main():
             a, c = row["after_20_steps"]["as_written"], row["after_20_steps"]["composed"]
             print(f"cfg {cfg} {w.name:34s} {riemann:4s}  as written {a['operations']:8.1f} ops {a['slots']:8.1f} slots | "
                   f"composed {c['operations']:8.1f} ops {c['slots']:8.1f} slots   (t=0: {row['initial_state']['composed']['slots']:.1f})")
-    doc = {"command": "python -m oracle.count_ops", "classes": CLASSES,
+    doc = {"command": "python tests/count_ops.py", "classes": CLASSES,
            "slot_weights": "fp32: div 6, sqrt 5; fp64: div 8, sqrt 10; neg 0; everything else 1 (DESIGN.md §8)", "rows": table}
     os.makedirs(os.path.join(ROOT, "profiles"), exist_ok=True)
     with open(os.path.join(ROOT, "profiles", "r3_counted_ops.json"), "w") as f:
         json.dump(doc, f, indent=1)
     with open(os.path.join(ROOT, "profiles", "r3_counted_ops.md"), "w") as f:
         f.write("# Counted arithmetic per cell per RK2 step, from the oracle instantiated with a counting scalar\n\n"
-                "Command: `python -m oracle.count_ops` (oracle/count_ops.cpp + oracle/count_ops.py; calls only oracle/ and "
+                "Command: `python tests/count_ops.py` (oracle/count_ops.cpp + tests/count_ops.py; calls only oracle/ and "
                 "the seeded input generators).  State 20 oracle steps after the recipe's initial condition, reduced grids.\n"
                 "`slots` = operations with a division / square root weighted by the kernels' fma sequence "
                 "(fp32 6 / 5, fp64 8 / 10); selects are not visible to a scalar type.\n\n"

@@ -715,3 +715,25 @@ def test_k_pack_is_deterministic_under_full_occupancy(gpu, name, n, dtype, opts,
                 assert h.stats() == 0 and np.isfinite(first).all()
             else:
                 assert np.array_equal(got, first), (name, rep)
+
+
+def test_binding_orders_a_temporary_torch_source_before_a_side_stream_handle(gpu, oracle_mod):
+    """set_state is asynchronous for a device source.  With the handle on a non-default stream, a temporary
+    `torch.from_numpy(U).cuda()` (a) is produced on torch's current stream, which the handle's stream must wait for,
+    and (b) would go back to torch's caching allocator - and be overwritten by the next allocation - before the copy
+    has run, unless the binding keeps it alive.  The wrapper does both (binding.ParaisoHydro._source)."""
+    import torch
+
+    w = inputs.random_smooth((512, 384), np.float32, seed=8)
+    ref, rdt = oracle_steps(oracle_mod, w, 2)
+    side = torch.cuda.Stream()
+    for _ in range(5):
+        with gpu.ParaisoHydro(w.n, w.extent, w.gamma, w.dtype, w.boundary, "hllc", stream=side) as h:
+            h.set_state(torch.from_numpy(w.U).cuda())  # a temporary: nothing else holds it
+            junk = [torch.full((w.U.size,), float("nan"), device="cuda") for _ in range(4)]  # would reuse its block
+            for k in range(2):
+                h.step(h.cfl_dt(w.cfl))
+            got = h.get_state()
+            assert h.stats() == 0
+            del junk
+        assert np.array_equal(got, ref)
